@@ -1,0 +1,7 @@
+"""B200-native brute-force incoherent de-dispersion (arxiv 1111.6399, ARTEMIS hot path).
+
+``out[d][t] = sum_c in[c][t + s(c,d)]`` for every trial DM of a plan (§2).
+The product is the C-ABI library ``libdedisp_b200.so`` (``include/dedisp.h``); this
+package is its thin ctypes binding plus the config/synthetic-input modules.
+"""
+from .configs import CONFIGS, SurveyConfig, shrink  # noqa: F401
