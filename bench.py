@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line per run (contract in the task statement).
+
+A step = one pass of the whole hot path (shifted accumulate over all channels for every DM trial
+of the plan; the shift table is built once per plan, outside the timed region, as the method
+does) over one synthetic batch of the workload. Default workload: c3, the MeerKAT-like fp32 config
+that carries BASELINE.json's roofline target. Metric: Gadds/s, one add per (DM, channel, sample).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "dedispersion Gadds/s (DM x chan x sample)"
+UNIT = "Gadds/s"
+N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 128 FP32/INT32 add lanes
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p.get("hbm_gbs", 6650.0)), float(p.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=fd, stderr=subprocess.DEVNULL)
+            os.close(fd)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        with open(self.path) as f:
+            for line in f:
+                tok = [t.strip() for t in line.split(",")]
+                if len(tok) < 9:
+                    continue
+                try:
+                    sm.append(float(tok[1])); mx.append(float(tok[2])); pw.append(float(tok[3]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, tok[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        os.unlink(self.path)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, target_s: float = 15.0):
+    """Time the oracle, as it stands, single-threaded, on a bounded row subset of the workload."""
+    import numpy as np
+    import oracle
+    from paper_1111_6399_b200 import synth
+    dm = cfg.dm_list()
+    tab = oracle.shift_table(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, dm)
+    nsamp_in = cfg.nsamp_out + int(tab.max())
+    x, _ = synth.make_input(cfg, tab, nsamp_in, device="cpu")
+    x = x.numpy()
+    rate_guess = {"f32": 1.0e9, "u8": 2.0e9, "f16": 0.1e9}[cfg.dtype]
+    per_row = cfg.nchans * cfg.nsamp_out
+    nrows = int(max(1, min(cfg.ndm, round(target_s * rate_guess / per_row))))
+    rows = np.linspace(0, cfg.ndm - 1, nrows).round().astype(np.int32)
+
+    def run():
+        t0 = time.perf_counter()
+        oracle.dedisperse(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, dm, x, cfg.nsamp_out, rows=rows)
+        return time.perf_counter() - t0
+
+    return run, nrows * per_row, f"{nrows} of {cfg.ndm} DM rows (evenly spread) x all {cfg.nchans} channels x all " \
+                                 f"{cfg.nsamp_out} samples of {cfg.name}, single thread"
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    run, adds, sample = oracle_sample(cfg, target_s=8.0)
+    for _ in range(args.warmup):
+        run()
+    times = [run() for _ in range(args.steps)]
+    tot = sum(times)
+    val = adds * args.steps / tot / 1e9
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic", "impl": "reference",
+            "config": {"workload": cfg.name, "nchans": cfg.nchans, "ndm": cfg.ndm, "nsamp_out": cfg.nsamp_out,
+                       "note": "oracle/ (plain C++ triple loop) on the host; each step = the bounded sample"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per dedisp_execute from the committed ncu --set full
+# capture (profiles/), keyed by (workload, resolved kernel); None until captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product has no CPU path"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    hbm_gbs, sm_max_mhz, peak_src = _peaks()
+    plan = P.Plan.from_config(cfg)                      # table build + upload: once per plan, not per step
+    if args.kernel:
+        plan.set_kernel({"naive": 1, "tiled": 2, "subband": 3}[args.kernel])
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    # each rank de-disperses its own beam (independent problems, no data-path collective): weak scaling
+    x, _ = synth.make_input(cfg, plan.shifts(), nsamp_in, device="cuda", seed=cfg.seed + 7919 * rank)
+    out = plan.alloc_out(cfg.nsamp_out)
+    adds = cfg.ndm * cfg.nchans * cfg.nsamp_out
+    launches = plan.launches_per_execute
+    stream = torch.cuda.current_stream()
+
+    for _ in range(args.warmup):
+        plan.execute(x, cfg.nsamp_out, out)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    for a, b in evs:                                    # input (4.4 GB for c3) >> 126 MB L2: no flush needed
+        a.record(stream)
+        plan.execute(x, cfg.nsamp_out, out)
+        b.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks(evs[0][0].elapsed_time(evs[-1][1]))
+    step_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps       # device time of one execute
+    value = world * adds * args.steps / (total_ms * 1e-3) / 1e9
+
+    # ---- e2e: the host-buffer C-ABI call; H2D + kernels + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        esteps = max(1, min(args.steps, args.e2e_steps))
+        h_in = torch.empty((cfg.nchans, nsamp_in), dtype=x.dtype, pin_memory=True)
+        h_in.copy_(x)
+        h_out = torch.empty((cfg.ndm, cfg.nsamp_out), dtype=out.dtype, pin_memory=True)
+        plan.execute_host(h_in, cfg.nsamp_out, h_out)   # warm-up: allocates the scratch
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(esteps):
+            plan.execute_host(h_in, cfg.nsamp_out, h_out)
+        barrier()
+        et = max_over_ranks(time.perf_counter() - t0)
+        e2e = {"value": world * adds * esteps / et / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
+               "d2h_bytes_per_step": h_out.numel() * h_out.element_size(), "steps": esteps,
+               "ms_per_step": 1e3 * et / esteps, "api": "dedisp_execute_host (pinned host buffers)"}
+        del h_in, h_out
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6 / 1e9            # Gadds/s at the max SM clock
+    achieved = adds / (step_ms * 1e-3) / 1e9
+    esize = cfg.esize
+    bytes_once = cfg.nchans * nsamp_in * esize + cfg.ndm * cfg.nsamp_out * 4
+    kname = {1: "naive", 2: "tiled", 3: "subband"}[plan.kernel]
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kname)),
+                "kernel": f"dedisp_{kname}_kernel", "launches_per_step": launches,
+                "peak_source": f"148 SMs x 128 lanes x sm_max_mhz ({peak_src} MEASURED_PEAKS.json clock)",
+                "hbm_bytes_once": bytes_once, "hbm_time_ms_at_peak": bytes_once / (hbm_gbs * 1e9) * 1e3,
+                "hbm_achieved_gbs": bytes_once / (step_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs}
+    if clocks and clocks.get("sm_mhz"):
+        roofline["frac_at_sampled_clock"] = achieved / (N_SM * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e9)
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        run, sadds, sample = oracle_sample(cfg, target_s=args.cpu_seconds)
+        dt = run()
+        cpu_baseline = {"value": sadds / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                        "seconds": dt}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "i32" if cfg.dtype == "u8" else "f32",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "nchans": cfg.nchans, "ndm": cfg.ndm, "nsamp_out": cfg.nsamp_out,
+                       "nsamp_in": nsamp_in, "in_dtype": cfg.dtype, "beams_per_gpu": 1,
+                       "l2": "input larger than L2, no flush", "kernel": kname,
+                       "parallelism": f"{world} independent beams, one per GPU, no collective"},
+            "real_time_factor": cfg.nsamp_out * cfg.tsamp / (total_ms / args.steps * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches * args.steps,
+            "roofline": roofline, "cpu_baseline": cpu_baseline}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--kernel", default=None, choices=["naive", "tiled", "subband"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    from paper_1111_6399_b200 import CONFIGS
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

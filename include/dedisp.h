@@ -1,0 +1,160 @@
+/* dedisp.h — C ABI of libdedisp_b200: brute-force incoherent de-dispersion on one B200 (sm_100a).
+ *
+ * The operation (§2: "shifting each frequency channel by the appropriate amount of
+ * time for each DM being searched" ... "before frequency integration"; formula fixed by
+ * BASELINE.json:north_star, readings R1-R10 in DESIGN.md):
+ *
+ *     out[d][t] = sum_{c=0}^{nchans-1} in[c][ t + s(c,d) ]        0 <= d < ndm, 0 <= t < nsamp_out
+ *     s(c,d)    = floor( 4.148808e3 * DM_d * (f_c^-2 - f_top^-2) / tsamp + 0.5 )
+ *
+ * evaluated in IEEE double on the host; f_c = fch1 + c*foff (MHz, foff < 0), f_top = fch1,
+ * tsamp in seconds. Input is channel-major with time contiguous (Fig. 2 caption:
+ * "cache-lines of constant frequency, contiguous time"). Every (d,c,t) term is added — the
+ * method is brute force, nothing is approximated or shared between trials.
+ *
+ * Conventions for every entry point:
+ *   - returns a dedisp_status; no exception or abort crosses the ABI;
+ *   - pointers named h_* are HOST memory, d_* are DEVICE memory of the current CUDA device;
+ *   - the caller owns every buffer it passes in; the plan owns its own host and device tables;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - there is no CPU fallback: on a machine without an sm_100 GPU plan creation fails with
+ *     DEDISP_EUNSUPPORTED / DEDISP_ECUDA (except DEDISP_PLAN_HOST_ONLY plans, which can only be
+ *     inspected, never executed).
+ */
+#ifndef DEDISP_B200_H
+#define DEDISP_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dedisp_plan dedisp_plan;     /* opaque */
+typedef struct dedisp_stream dedisp_stream; /* opaque: streaming multi-beam driver */
+
+enum dedisp_dtype { DEDISP_U8 = 0, DEDISP_F16 = 1, DEDISP_F32 = 2 };
+
+enum dedisp_status {
+    DEDISP_OK = 0,
+    DEDISP_EINVAL = 1,       /* bad argument (see each call) */
+    DEDISP_ENOMEM = 2,       /* host or device allocation failed */
+    DEDISP_ECUDA = 3,        /* a CUDA call failed; text via dedisp_last_cuda_error */
+    DEDISP_EUNSUPPORTED = 4  /* device is not sm_100, or maxshift >= 2^31, or plan is host-only */
+};
+
+/* Kernel selection (dedisp_plan_set_kernel). AUTO picks SUBBAND when the plan admits it, else TILED.
+ * NAIVE is the one-thread-per-(d,t) cross-check kernel used by the parity tests' chain of trust. */
+enum dedisp_kernel {
+    DEDISP_KERNEL_AUTO = 0,
+    DEDISP_KERNEL_NAIVE = 1,   /* global loads through L1, no staging */
+    DEDISP_KERNEL_TILED = 2,   /* CTA = DM tile x time tile, channel windows staged in shared memory */
+    DEDISP_KERNEL_SUBBAND = 3  /* exact sub-band re-skewed multi-pass with register-window reuse */
+};
+
+enum dedisp_plan_flags {
+    DEDISP_PLAN_DEFAULT = 0,
+    DEDISP_PLAN_HOST_ONLY = 1  /* build host tables only; no CUDA call is made; execute -> EUNSUPPORTED */
+};
+
+/* ---- subsystem (2): shift-table builder ("the shifting value
+ * is calculated using as few operations as possible" — here: once per plan, on the host, in double).
+ *
+ * dedisp_shift_table_host: pure host function, no CUDA. Writes s(c,d) to h_table[c*ndm + d]
+ * (int32) and the maximum to *h_maxshift (may be NULL). EINVAL on nchans<1, ndm<1, tsamp<=0,
+ * fch1<=0, foff>=0, lowest channel frequency <=0, DM negative / non-finite / decreasing, NULLs;
+ * EUNSUPPORTED if any shift >= 2^31. */
+int dedisp_shift_table_host(int nchans, double fch1_mhz, double foff_mhz, double tsamp_s,
+                            const double *h_dm_list, int ndm, int *h_table, long long *h_maxshift);
+
+/* ---- subsystem (1): plan / execute / destroy (BASELINE.json:north_star (1)).
+ *
+ * dedisp_plan_create: validates (same rules as dedisp_shift_table_host, plus in_dtype), builds the
+ * shift table and the kernels' tiling/sub-band metadata on the host, uploads them to the current
+ * device. h_dm_list[ndm] is copied. in_dtype is a dedisp_dtype. */
+int dedisp_plan_create(dedisp_plan **plan, int nchans, double fch1_mhz, double foff_mhz,
+                       double tsamp_s, const double *h_dm_list, int ndm, int in_dtype);
+int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1_mhz, double foff_mhz,
+                          double tsamp_s, const double *h_dm_list, int ndm, int in_dtype,
+                          unsigned flags);
+
+/* dedisp_execute: out[d][t] for all ndm trials and 0 <= t < nsamp_out, asynchronously on `stream`.
+ *   d_in : [nchans][nsamp_out + maxshift] elements of in_dtype, dense rows (row stride =
+ *          nsamp_out + dedisp_plan_max_shift(plan)); channel 0 = fch1 (highest frequency).
+ *   d_out: [ndm][nsamp_out], row stride nsamp_out; int32 for DEDISP_U8 input (exact), float32 for
+ *          DEDISP_F16 / DEDISP_F32 input (fp32 accumulation; summation order unspecified).
+ * Allocates nothing. May be called repeatedly; concurrent calls on different streams are allowed
+ * (the plan is read-only after create / set_kernel). EINVAL: NULLs, nsamp_out < 1. */
+int dedisp_execute(dedisp_plan *plan, const void *d_in, long long nsamp_out, void *d_out,
+                   void *stream);
+
+/* Same with explicit row strides in ELEMENTS (in_stride >= nsamp_out + maxshift, out_stride >=
+ * nsamp_out), else EINVAL. A 16-byte-aligned d_in and in_stride*elemsize let the staging use
+ * 16-byte transactions; any stride is correct. */
+int dedisp_execute_strided(dedisp_plan *plan, const void *d_in, long long in_stride_elems,
+                           long long nsamp_out, void *d_out, long long out_stride_elems,
+                           void *stream);
+
+/* Beam batching (north_star (4) "batches beams"): nbeams independent inputs through one plan in one
+ * launch. Beam b reads d_in + b*in_beam_stride_elems and writes d_out + b*out_beam_stride_elems
+ * (ELEMENTS of the input / output type); each beam is laid out as in dedisp_execute_strided.
+ * EINVAL: nbeams < 1 or > 65535, beam strides smaller than one beam's extent. */
+int dedisp_execute_batched(dedisp_plan *plan, int nbeams, const void *d_in, long long in_stride_elems,
+                           long long in_beam_stride_elems, long long nsamp_out, void *d_out,
+                           long long out_stride_elems, long long out_beam_stride_elems, void *stream);
+
+/* Host-buffer convenience (the end-to-end call bench.py's "e2e" times): h_in [nchans][nsamp_out +
+ * maxshift] and h_out [ndm][nsamp_out] are HOST buffers (pinned memory makes the copies
+ * asynchronous to the host and full speed). Copies the input to plan-owned device scratch (grown
+ * on demand, freed at destroy), executes, copies the result back and SYNCHRONISES `stream` before
+ * returning. Not re-entrant per plan (the scratch is shared). */
+int dedisp_execute_host(dedisp_plan *plan, const void *h_in, long long nsamp_out, void *h_out,
+                        void *stream);
+
+int dedisp_plan_destroy(dedisp_plan *plan); /* NULL is OK */
+
+/* ---- inspection */
+long long dedisp_plan_max_shift(const dedisp_plan *plan); /* nsamp_in = nsamp_out + this; -1 on NULL */
+int dedisp_plan_nchans(const dedisp_plan *plan);
+int dedisp_plan_ndm(const dedisp_plan *plan);
+/* Copies the plan's table to h_out[nchans*ndm] (index c*ndm + d). For the table-parity test. */
+int dedisp_plan_get_shifts(const dedisp_plan *plan, int *h_out);
+/* Force a kernel (enum dedisp_kernel). EUNSUPPORTED if the plan does not admit it. */
+int dedisp_plan_set_kernel(dedisp_plan *plan, int kernel);
+/* The kernel dedisp_execute will launch for this plan (resolved, never AUTO). */
+int dedisp_plan_get_kernel(const dedisp_plan *plan);
+/* Sub-band layout of the SUBBAND kernel: number of passes G (0 if the plan has none) and, if
+ * h_first_chan != NULL, the G+1 channel boundaries. */
+int dedisp_plan_num_subbands(const dedisp_plan *plan);
+int dedisp_plan_get_subbands(const dedisp_plan *plan, int *h_first_chan /* [G+1] */);
+/* Host check used by the CPU tests: rebuild s(c,d) for every (c,d) from the SUBBAND kernel's packed
+ * per-(pass, DM group, channel) records and compare with the shift table. Returns the number of
+ * mismatching entries (0 = the records encode exactly the table), or -1 if the plan has none. */
+long long dedisp_plan_verify_records(const dedisp_plan *plan);
+/* Number of kernel launches one dedisp_execute issues for this plan (for bench.py's gpu_launches). */
+int dedisp_plan_launches_per_execute(const dedisp_plan *plan);
+
+const char *dedisp_error_string(int code);
+const char *dedisp_last_cuda_error(const dedisp_plan *plan);
+
+/* ---- subsystem (4): streaming multi-beam driver (the paper's MDSM
+ * wrapper). Input chunk k holds samples [k*N, (k+1)*N) of every (beam, channel);
+ * output block k holds out[.][t] for global t in [k*N - maxshift, (k+1)*N - maxshift): the history
+ * before the first chunk is zero, so the first maxshift outputs of block 0 are warm-up.
+ * Equivalent to one dedisp_execute over the whole stream delayed by maxshift.
+ *
+ * dedisp_stream_create: device buffers for nbeams x nchans x (maxshift + chunk) input (nbuffers
+ * copies, >= 2, for copy/compute overlap) and nbeams x ndm x chunk output per buffer; one copy
+ * stream, one compute stream. The plan must outlive the stream object. */
+int dedisp_stream_create(dedisp_stream **s, dedisp_plan *plan, int nbeams, long long chunk_nsamp,
+                         int nbuffers);
+/* dedisp_stream_push: enqueue one chunk. h_chunk: host memory (pinned for true async copies),
+ * layout [beam][chan][chunk_nsamp] of the plan's in_dtype. Returns immediately; *d_out (device,
+ * [beam][ndm][chunk_nsamp], owned by the stream object, reused after nbuffers pushes) is valid
+ * once *done_event (a cudaEvent_t as void*) has completed or after dedisp_stream_sync. */
+int dedisp_stream_push(dedisp_stream *s, const void *h_chunk, void **d_out, void **done_event);
+int dedisp_stream_sync(dedisp_stream *s);
+int dedisp_stream_destroy(dedisp_stream *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_B200_H */

@@ -5,3 +5,5 @@ The product is the C-ABI library ``libdedisp_b200.so`` (``include/dedisp.h``); t
 package is its thin ctypes binding plus the config/synthetic-input modules.
 """
 from .configs import CONFIGS, SurveyConfig, shrink  # noqa: F401
+from .api import (Plan, Stream, DedispError, shift_table_host, lib,  # noqa: F401,E402
+                  KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND)

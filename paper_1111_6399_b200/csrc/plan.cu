@@ -1,0 +1,229 @@
+// plan.cu — subsystem (1): the C ABI of include/dedisp.h (plan create / execute / destroy and
+// inspection). Host logic only; kernels live in kernels_tiled.cu and subband.cu.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "plan.h"
+
+namespace {
+
+int fail_cuda(dedisp_plan *p, cudaError_t e, const char *what) {
+    if (p) p->cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA;
+}
+
+int resolve_kernel(const dedisp_plan *p) {
+    int k = p->kernel;
+    if (k == DEDISP_KERNEL_AUTO) k = p->sb.ok ? DEDISP_KERNEL_SUBBAND : p->tiled.ok ? DEDISP_KERNEL_TILED : DEDISP_KERNEL_NAIVE;
+    return k;
+}
+
+}  // namespace
+
+int execute_impl(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
+                 long long out_stride, Batch b, cudaStream_t st) {
+    if (!p || !d_in || !d_out || nsamp_out < 1) return DEDISP_EINVAL;
+    if (in_stride < nsamp_out + p->maxshift || out_stride < nsamp_out) return DEDISP_EINVAL;
+    if (p->flags & DEDISP_PLAN_HOST_ONLY) return DEDISP_EUNSUPPORTED;
+    if (nsamp_out + p->maxshift >= (1ll << 40)) return DEDISP_EUNSUPPORTED;
+    int k = resolve_kernel(p);
+    // the staged kernels align window starts down to 16 B relative to an aligned base
+    if (((uintptr_t)d_in & 15) != 0 && k != DEDISP_KERNEL_NAIVE) {
+        if (p->kernel != DEDISP_KERNEL_AUTO) return DEDISP_EINVAL;
+        k = DEDISP_KERNEL_NAIVE;
+    }
+    cudaError_t e;
+    switch (k) {
+        case DEDISP_KERNEL_SUBBAND: e = launch_subband(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
+        case DEDISP_KERNEL_TILED: e = launch_tiled(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
+        default: e = launch_naive(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
+    }
+    if (e != cudaSuccess) return fail_cuda(p, e, "kernel launch");
+    return DEDISP_OK;
+}
+
+extern "C" {
+
+int dedisp_shift_table_host(int nchans, double fch1, double foff, double tsamp, const double *h_dm_list, int ndm,
+                            int *h_table, long long *h_maxshift) {
+    return build_shift_table(nchans, fch1, foff, tsamp, h_dm_list, ndm, h_table, h_maxshift);
+}
+
+int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1, double foff, double tsamp,
+                          const double *h_dm_list, int ndm, int in_dtype, unsigned flags) {
+    if (!plan) return DEDISP_EINVAL;
+    *plan = nullptr;
+    if (in_dtype != DEDISP_U8 && in_dtype != DEDISP_F16 && in_dtype != DEDISP_F32) return DEDISP_EINVAL;
+    if (nchans < 1 || ndm < 1 || !h_dm_list) return DEDISP_EINVAL;
+    if ((double)nchans * (double)ndm > 2.0e9) return DEDISP_EUNSUPPORTED;
+    dedisp_plan *p = new (std::nothrow) dedisp_plan();
+    if (!p) return DEDISP_ENOMEM;
+    int rc = DEDISP_OK;
+    try {
+        p->nchans = nchans; p->ndm = ndm; p->dtype = in_dtype;
+        p->fch1 = fch1; p->foff = foff; p->tsamp = tsamp; p->flags = flags;
+        p->dm.assign(h_dm_list, h_dm_list + ndm);
+        p->shifts.resize((size_t)nchans * ndm);
+        rc = build_shift_table(nchans, fch1, foff, tsamp, p->dm.data(), ndm, p->shifts.data(), &p->maxshift);
+        if (rc == DEDISP_OK && in_dtype == DEDISP_U8 && (double)nchans * 255.0 > 2147483647.0) rc = DEDISP_EUNSUPPORTED;
+        if (rc == DEDISP_OK) {
+            tiled_choose_geom(p);
+            subband_build(p);
+        }
+    } catch (const std::bad_alloc &) {
+        rc = DEDISP_ENOMEM;
+    }
+    if (rc != DEDISP_OK) { delete p; return rc; }
+
+    if (!(flags & DEDISP_PLAN_HOST_ONLY)) {
+        cudaError_t e = cudaGetDevice(&p->device);
+        if (e != cudaSuccess) { rc = fail_cuda(nullptr, e, "cudaGetDevice"); delete p; return rc; }
+        cudaDeviceProp prop;
+        e = cudaGetDeviceProperties(&prop, p->device);
+        if (e != cudaSuccess) { delete p; return DEDISP_ECUDA; }
+        if (prop.major != 10) { delete p; return DEDISP_EUNSUPPORTED; }  // sm_100a cubin only, no fallback
+        p->sm_count = prop.multiProcessorCount;
+        const size_t bytes = p->shifts.size() * sizeof(int32_t);
+        e = cudaMalloc(&p->d_shifts, bytes);
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_shifts, p->shifts.data(), bytes, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = subband_upload(p);
+        if (e != cudaSuccess) {
+            rc = fail_cuda(nullptr, e, "plan upload");
+            dedisp_plan_destroy(p);
+            return rc;
+        }
+    }
+    *plan = p;
+    return DEDISP_OK;
+}
+
+int dedisp_plan_create(dedisp_plan **plan, int nchans, double fch1, double foff, double tsamp,
+                       const double *h_dm_list, int ndm, int in_dtype) {
+    return dedisp_plan_create_ex(plan, nchans, fch1, foff, tsamp, h_dm_list, ndm, in_dtype, DEDISP_PLAN_DEFAULT);
+}
+
+int dedisp_execute_strided(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,
+                           void *d_out, long long out_stride, void *stream) {
+    return execute_impl(p, d_in, in_stride, nsamp_out, d_out, out_stride, Batch(), (cudaStream_t)stream);
+}
+
+int dedisp_execute(dedisp_plan *p, const void *d_in, long long nsamp_out, void *d_out, void *stream) {
+    if (!p) return DEDISP_EINVAL;
+    return execute_impl(p, d_in, nsamp_out + p->maxshift, nsamp_out, d_out, nsamp_out, Batch(), (cudaStream_t)stream);
+}
+
+int dedisp_execute_batched(dedisp_plan *p, int nbeams, const void *d_in, long long in_stride,
+                           long long in_beam_stride, long long nsamp_out, void *d_out, long long out_stride,
+                           long long out_beam_stride, void *stream) {
+    if (!p || nbeams < 1 || nbeams > 65535) return DEDISP_EINVAL;
+    if (in_beam_stride < (long long)p->nchans * in_stride - (in_stride - nsamp_out - p->maxshift)) return DEDISP_EINVAL;
+    if (out_beam_stride < (long long)p->ndm * out_stride - (out_stride - nsamp_out)) return DEDISP_EINVAL;
+    Batch b;
+    b.n = nbeams; b.in_stride = in_beam_stride; b.out_stride = out_beam_stride;
+    return execute_impl(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, (cudaStream_t)stream);
+}
+
+int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, void *h_out, void *stream) {
+    if (!p || !h_in || !h_out || nsamp_out < 1) return DEDISP_EINVAL;
+    if (p->flags & DEDISP_PLAN_HOST_ONLY) return DEDISP_EUNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long nsamp_in = nsamp_out + p->maxshift;
+    const size_t in_bytes = (size_t)p->nchans * nsamp_in * dtype_esize(p->dtype);
+    const size_t out_bytes = (size_t)p->ndm * nsamp_out * 4;
+    cudaError_t e = cudaSuccess;
+    if (in_bytes > p->host_in_bytes) {
+        if (p->d_host_in) cudaFree(p->d_host_in);
+        p->d_host_in = nullptr; p->host_in_bytes = 0;
+        e = cudaMalloc(&p->d_host_in, in_bytes);
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host input scratch");
+        p->host_in_bytes = in_bytes;
+    }
+    if (out_bytes > p->host_out_bytes) {
+        if (p->d_host_out) cudaFree(p->d_host_out);
+        p->d_host_out = nullptr; p->host_out_bytes = 0;
+        e = cudaMalloc(&p->d_host_out, out_bytes);
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host output scratch");
+        p->host_out_bytes = out_bytes;
+    }
+    e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
+    const int rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+    if (rc != DEDISP_OK) return rc;
+    e = cudaMemcpyAsync(h_out, p->d_host_out, out_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host D2H");
+    return DEDISP_OK;
+}
+
+int dedisp_plan_destroy(dedisp_plan *p) {
+    if (!p) return DEDISP_OK;
+    if (p->d_shifts) cudaFree(p->d_shifts);
+    if (p->d_host_in) cudaFree(p->d_host_in);
+    if (p->d_host_out) cudaFree(p->d_host_out);
+    subband_free(p);
+    delete p;
+    return DEDISP_OK;
+}
+
+long long dedisp_plan_max_shift(const dedisp_plan *p) { return p ? p->maxshift : -1; }
+int dedisp_plan_nchans(const dedisp_plan *p) { return p ? p->nchans : -1; }
+int dedisp_plan_ndm(const dedisp_plan *p) { return p ? p->ndm : -1; }
+
+int dedisp_plan_get_shifts(const dedisp_plan *p, int *h_out) {
+    if (!p || !h_out) return DEDISP_EINVAL;
+    std::memcpy(h_out, p->shifts.data(), p->shifts.size() * sizeof(int32_t));
+    return DEDISP_OK;
+}
+
+int dedisp_plan_set_kernel(dedisp_plan *p, int kernel) {
+    if (!p) return DEDISP_EINVAL;
+    switch (kernel) {
+        case DEDISP_KERNEL_AUTO:
+        case DEDISP_KERNEL_NAIVE: break;
+        case DEDISP_KERNEL_TILED: if (!p->tiled.ok) return DEDISP_EUNSUPPORTED; break;
+        case DEDISP_KERNEL_SUBBAND: if (!p->sb.ok) return DEDISP_EUNSUPPORTED; break;
+        default: return DEDISP_EINVAL;
+    }
+    p->kernel = kernel;
+    return DEDISP_OK;
+}
+
+int dedisp_plan_get_kernel(const dedisp_plan *p) { return p ? resolve_kernel(p) : -1; }
+
+int dedisp_plan_num_subbands(const dedisp_plan *p) {
+    if (!p) return -1;
+    return p->sb.ok ? (int)p->sb.first_chan.size() - 1 : 0;
+}
+
+int dedisp_plan_get_subbands(const dedisp_plan *p, int *h_first_chan) {
+    if (!p || !h_first_chan) return DEDISP_EINVAL;
+    if (!p->sb.ok) return DEDISP_EUNSUPPORTED;
+    std::memcpy(h_first_chan, p->sb.first_chan.data(), p->sb.first_chan.size() * sizeof(int));
+    return DEDISP_OK;
+}
+
+long long dedisp_plan_verify_records(const dedisp_plan *p) {
+    if (!p || !p->sb.ok) return -1;
+    return subband_verify_records(p);
+}
+
+int dedisp_plan_launches_per_execute(const dedisp_plan *p) {
+    if (!p) return -1;
+    return resolve_kernel(p) == DEDISP_KERNEL_SUBBAND ? (int)p->sb.first_chan.size() - 1 : 1;
+}
+
+const char *dedisp_error_string(int code) {
+    switch (code) {
+        case DEDISP_OK: return "ok";
+        case DEDISP_EINVAL: return "invalid argument";
+        case DEDISP_ENOMEM: return "out of memory";
+        case DEDISP_ECUDA: return "CUDA error";
+        case DEDISP_EUNSUPPORTED: return "unsupported (device is not sm_100, shift >= 2^31, host-only plan, or kernel not admitted by the plan)";
+        default: return "unknown error code";
+    }
+}
+
+const char *dedisp_last_cuda_error(const dedisp_plan *p) { return p ? p->cuda_err.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,87 @@
+"""CPU-only checks of the C-ABI library: it loads without a GPU, exports every symbol that
+include/dedisp.h declares, its host shift-table builder agrees with the ORACLE's independent
+table on every entry of all five configs, and host-side validation returns the documented codes.
+No compute call is made here.
+"""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1111_6399_b200 as P
+from paper_1111_6399_b200 import CONFIGS, api
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dedisp.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dedisp_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    declared = _declared_symbols()
+    assert len(declared) >= 20
+    L = api.lib()
+    for name in declared:
+        assert hasattr(L, name), f"{name} declared in include/dedisp.h but not exported"
+    assert sorted(api.SYMBOLS) == declared, "binding's symbol list out of sync with the header"
+
+
+@pytest.mark.parametrize("name", list(CONFIGS))
+def test_library_shift_table_equals_oracle_table(name, golden):
+    cfg = CONFIGS[name]
+    tab, mx = P.shift_table_host(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list())
+    ref = oracle.shift_table(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list())
+    assert np.array_equal(tab.astype(np.int64), ref)
+    pins, _, _ = golden
+    assert mx == pins[name][0]                       # maxshift regression value (tests/golden/shift_pins.txt)
+
+
+def test_host_only_plan_inspection_and_refusal():
+    cfg = CONFIGS["c2"]
+    plan = P.Plan.from_config(cfg, host_only=True)
+    assert (plan.nchans, plan.ndm, plan.max_shift) == (496, 2000, 28324)
+    assert np.array_equal(plan.shifts().astype(np.int64),
+                          oracle.shift_table(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list()))
+    assert plan.kernel in (P.KERNEL_TILED, P.KERNEL_SUBBAND, P.KERNEL_NAIVE)
+    assert plan.launches_per_execute >= 1
+    # a host-only plan never executes, and there is no CPU fallback
+    rc = api.lib().dedisp_execute(plan._h, ctypes.c_void_p(16), 10, ctypes.c_void_p(16), None)
+    assert rc == api.EUNSUPPORTED
+
+
+def test_validation_codes():
+    L = api.lib()
+    dm = (ctypes.c_double * 3)(0.0, 1.0, 2.0)
+    tab = (ctypes.c_int * 12)()
+    mx = ctypes.c_longlong()
+    ok = lambda *a: L.dedisp_shift_table_host(*a, tab, ctypes.byref(mx))
+    assert ok(4, 100.0, -1.0, 1e-3, dm, 3) == api.OK
+    assert ok(0, 100.0, -1.0, 1e-3, dm, 3) == api.EINVAL
+    assert ok(4, 100.0, +1.0, 1e-3, dm, 3) == api.EINVAL      # ascending band
+    assert ok(4, 100.0, -1.0, 0.0, dm, 3) == api.EINVAL       # tsamp
+    assert ok(4, 3.0, -1.0, 1e-3, dm, 3) == api.EINVAL        # lowest channel <= 0 MHz
+    bad = (ctypes.c_double * 3)(0.0, 2.0, 1.0)
+    assert ok(4, 100.0, -1.0, 1e-3, bad, 3) == api.EINVAL     # decreasing DMs
+    nan = (ctypes.c_double * 3)(0.0, float("nan"), 1.0)
+    assert ok(4, 100.0, -1.0, 1e-3, nan, 3) == api.EINVAL
+    huge = (ctypes.c_double * 3)(0.0, 1.0, 1e9)
+    assert ok(4, 100.0, -20.0, 1e-9, huge, 3) == api.EUNSUPPORTED  # shift >= 2^31
+    h = ctypes.c_void_p()
+    assert L.dedisp_plan_create_ex(ctypes.byref(h), 4, 100.0, -1.0, 1e-3, dm, 3, 7, 1) == api.EINVAL  # dtype
+    assert L.dedisp_plan_destroy(None) == api.OK
+    assert L.dedisp_plan_max_shift(None) == -1
+    assert L.dedisp_error_string(api.ECUDA) == b"CUDA error"
+
+
+def test_no_gpu_means_loud_failure():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(P.DedispError):
+        P.Plan.from_config(CONFIGS["c1"])

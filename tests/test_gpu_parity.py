@@ -1,0 +1,181 @@
+"""-m gpu: CUDA path vs oracle, element by element, through the C ABI (include/dedisp.h).
+
+Chain of trust: oracle => every kernel on oracle-sized cases (full outputs) and on
+row subsets of the full-size configs; optimised kernels == NAIVE kernel on the FULL output of every
+full-size config (NAIVE is itself oracle-checked; it is a cross-check, never the oracle).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_1111_6399_b200 as P
+from paper_1111_6399_b200 import CONFIGS, shrink
+from paper_1111_6399_b200.configs import SurveyConfig
+
+from _util import assert_matches_oracle, make_case, oracle_table, oracle_rows, run_gpu, spread_rows
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [P.KERNEL_NAIVE, P.KERNEL_TILED, P.KERNEL_SUBBAND]
+KNAME = {P.KERNEL_NAIVE: "naive", P.KERNEL_TILED: "tiled", P.KERNEL_SUBBAND: "subband"}
+
+
+def _plan_with(cfg, kernel):
+    plan = P.Plan.from_config(cfg)
+    try:
+        plan.set_kernel(kernel)
+    except P.DedispError as e:
+        assert e.code == 4
+        pytest.skip(f"{KNAME[kernel]} kernel not admitted by plan {cfg.name}")
+    return plan
+
+
+# ---- oracle-sized cases: full outputs, several tiles plus ragged tails in both d and t
+SMALL = {
+    "c1": CONFIGS["c1"],
+    "c2s": shrink(CONFIGS["c2"], nsamp_out=5000, ndm_stride=9),          # 223 DMs, u8, shifts to 28k
+    "c3s": shrink(CONFIGS["c3"], nchans=300, nsamp_out=4500, ndm_stride=31),
+    "c4s": shrink(CONFIGS["c4"], nchans=257, nsamp_out=3100, ndm_stride=29),
+    "c5s": shrink(CONFIGS["c5"], nchans=128, nsamp_out=2049, ndm_stride=5),
+    "fine": SurveyConfig("fine_dm_u8", 200, 159.0, -32.0 / 200.0, 327.68e-6, 3000, ((0.0, 0.01, 333),),
+                         "u8", 128.0, 16.0, 20.0, 2, 77),                  # paper regime: adjacent-DM delta <= 1
+}
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=[KNAME[k] for k in KERNELS])
+@pytest.mark.parametrize("name", list(SMALL))
+def test_small_full_output_vs_oracle(name, kernel):
+    cfg = SMALL[name]
+    plan = _plan_with(cfg, kernel)
+    x, tab, _ = make_case(cfg)
+    assert plan.max_shift == int(tab.max())
+    out, _ = run_gpu(cfg, x, kernel, plan=plan)
+    ref = oracle_rows(cfg, x.cpu().numpy())
+    assert_matches_oracle(cfg, out, ref, what=f"{name}/{KNAME[kernel]}")
+
+
+def test_c1_pulse_recovered():
+    """PAPER.md:52 (Fig. 3): the injected pulse is recovered at its DM and time."""
+    cfg = CONFIGS["c1"]
+    x, tab, pulses = make_case(cfg, noise=False)
+    out, _ = run_gpu(cfg, x)
+    d_inj, t0 = pulses[0]
+    assert out[d_inj, t0].item() == cfg.nchans * cfg.pulse_amp
+    assert int(out.argmax()) == d_inj * cfg.nsamp_out + t0
+
+
+# ---- edge shapes
+EDGE = [
+    dict(nchans=1, ndm_seg=((0.0, 1.0, 5),), nsamp_out=100),
+    dict(nchans=7, ndm_seg=((3.0, 1.0, 1),), nsamp_out=1),
+    dict(nchans=33, ndm_seg=((0.0, 0.0, 9),), nsamp_out=513),            # all-zero DM list
+    dict(nchans=33, ndm_seg=((5.0, 0.0, 3), (5.0, 0.0, 2), (9.0, 2.0, 4)), nsamp_out=1025),  # duplicates
+    dict(nchans=64, ndm_seg=((0.0, 40.0, 17),), nsamp_out=777),          # coarse plan, wide windows
+]
+
+
+@pytest.mark.parametrize("dtype", ["u8", "f16", "f32"])
+@pytest.mark.parametrize("case", range(len(EDGE)))
+@pytest.mark.parametrize("kernel", KERNELS, ids=[KNAME[k] for k in KERNELS])
+def test_edge_shapes(case, dtype, kernel):
+    e = EDGE[case]
+    mean, sig = (128.0, 16.0) if dtype == "u8" else (0.0, 1.0)
+    cfg = SurveyConfig(f"edge{case}_{dtype}", e["nchans"], 400.0, -100.0 / max(e["nchans"], 2), 256e-6, e["nsamp_out"],
+                       e["ndm_seg"], dtype, mean, sig, 3.0, 1, 1000 + case)
+    plan = _plan_with(cfg, kernel)
+    x, tab, _ = make_case(cfg)
+    out, _ = run_gpu(cfg, x, kernel, plan=plan)
+    assert_matches_oracle(cfg, out, oracle_rows(cfg, x.cpu().numpy()), what=cfg.name)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=[KNAME[k] for k in KERNELS])
+def test_strided_and_batched(kernel):
+    """dedisp_execute_strided / _batched: padded pitches, 3 beams in one launch == per-beam oracle."""
+    cfg = SMALL["c5s"]
+    plan = _plan_with(cfg, kernel)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    pitch = nsamp_in + 13
+    xs = torch.zeros((3, cfg.nchans + 1, pitch), dtype=torch.uint8, device="cuda")
+    outs = torch.full((3, cfg.ndm + 2, cfg.nsamp_out + 5), -7, dtype=torch.int32, device="cuda")
+    hosts = []
+    for b in range(3):
+        x, _, _ = make_case(cfg, seed=500 + b)
+        xs[b, :cfg.nchans, :nsamp_in] = x
+        hosts.append(x.cpu().numpy())
+    plan.execute(xs[:, :cfg.nchans], cfg.nsamp_out, outs[:, :cfg.ndm])
+    torch.cuda.synchronize()
+    for b in range(3):
+        assert_matches_oracle(cfg, outs[b, :cfg.ndm, :cfg.nsamp_out], oracle_rows(cfg, hosts[b]), what=f"beam {b}")
+    assert bool((outs[:, cfg.ndm:] == -7).all()) and bool((outs[:, :, cfg.nsamp_out:] == -7).all())
+
+
+def test_errors():
+    cfg = CONFIGS["c1"]
+    plan = P.Plan.from_config(cfg)
+    x = torch.zeros((cfg.nchans, cfg.nsamp_out + plan.max_shift - 1), device="cuda")
+    with pytest.raises(P.DedispError) as ei:
+        plan.execute(x, cfg.nsamp_out)     # row too short
+    assert ei.value.code == 1
+    with pytest.raises(P.DedispError):
+        plan.set_kernel(99)
+    with pytest.raises(P.DedispError):
+        P.Plan(4, 100.0, +1.0, 1e-3, [0.0, 1.0], "f32")       # ascending band rejected (DESIGN R11)
+    with pytest.raises(P.DedispError):
+        P.Plan(4, 100.0, -1.0, 1e-3, [1.0, 0.5], "f32")       # decreasing DMs rejected
+
+
+# ---- full-size configs, in the launch configuration bench.py times
+def _full(name, nrows):
+    cfg = CONFIGS[name]
+    x, tab, pulses = make_case(cfg)
+    rows = spread_rows(cfg.ndm, nrows, extra=[p[0] for p in pulses])
+    return cfg, x, rows
+
+
+@pytest.mark.parametrize("name,nrows", [("c2", 48), ("c3", 12), ("c4", 8)])
+def test_full_size_rows_vs_oracle_and_naive(name, nrows):
+    cfg, x, rows = _full(name, nrows)
+    ref = oracle_rows(cfg, x.cpu().numpy(), rows=rows)
+    out_naive, plan = run_gpu(cfg, x, P.KERNEL_NAIVE)
+    assert_matches_oracle(cfg, out_naive, ref, rows=rows, what=f"{name}/naive")
+    for k in (P.KERNEL_TILED, P.KERNEL_SUBBAND, P.KERNEL_AUTO):
+        try:
+            plan.set_kernel(k)
+        except P.DedispError:
+            continue
+        out = plan.execute(x, cfg.nsamp_out)
+        torch.cuda.synchronize()
+        assert_matches_oracle(cfg, out, ref, rows=rows, what=f"{name}/kernel{k}")
+        if cfg.dtype == "u8":
+            assert torch.equal(out, out_naive)
+        else:
+            # different summation orders: both within 1e-5*sum|terms| of the oracle on the checked rows;
+            # on the full output bound their distance by the same scale (sum|terms| <= nchans * max|x|)
+            scale = 2e-5 * float(x.abs().max()) * cfg.nchans
+            assert float((out - out_naive).abs().max()) <= scale
+        del out
+    del out_naive
+    torch.cuda.empty_cache()
+
+
+def test_c5_one_chunk_batched_rows_vs_oracle():
+    """c5 launch shape: 32 beams x 1024 chans x (32768 + maxshift) u8 in one batched launch."""
+    cfg = CONFIGS["c5"]
+    plan = P.Plan.from_config(cfg)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    tab = oracle_table(cfg)
+    assert plan.max_shift == int(tab.max())
+    xs = torch.empty((cfg.nbeams, cfg.nchans, nsamp_in), dtype=torch.uint8, device="cuda")
+    from paper_1111_6399_b200 import synth
+    for b in range(cfg.nbeams):
+        xs[b], _ = synth.make_input(cfg, tab, nsamp_in, device="cuda", seed=cfg.seed * 1000003 + b * 101)
+    out = plan.execute(xs, cfg.nsamp_out)
+    torch.cuda.synchronize()
+    rows = spread_rows(cfg.ndm, 24)
+    for b in (0, 17, 31):
+        ref = oracle_rows(cfg, xs[b].cpu().numpy(), rows=rows)
+        assert_matches_oracle(cfg, out[b], ref, rows=rows, what=f"c5 beam {b}")
+    plan.set_kernel(P.KERNEL_NAIVE)
+    out2 = plan.execute(xs, cfg.nsamp_out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
