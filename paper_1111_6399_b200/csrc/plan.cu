@@ -193,13 +193,14 @@ int dedisp_plan_get_kernel(const dedisp_plan *p) { return p ? resolve_kernel(p) 
 
 int dedisp_plan_num_subbands(const dedisp_plan *p) {
     if (!p) return -1;
-    return p->sb.ok ? (int)p->sb.first_chan.size() - 1 : 0;
+    return p->sb.ok ? (int)p->sb.passes.size() : 0;
 }
 
 int dedisp_plan_get_subbands(const dedisp_plan *p, int *h_first_chan) {
     if (!p || !h_first_chan) return DEDISP_EINVAL;
     if (!p->sb.ok) return DEDISP_EUNSUPPORTED;
-    std::memcpy(h_first_chan, p->sb.first_chan.data(), p->sb.first_chan.size() * sizeof(int));
+    for (size_t g = 0; g < p->sb.passes.size(); ++g) h_first_chan[g] = p->sb.passes[g].c_begin;
+    h_first_chan[p->sb.passes.size()] = p->nchans;
     return DEDISP_OK;
 }
 
@@ -210,7 +211,7 @@ long long dedisp_plan_verify_records(const dedisp_plan *p) {
 
 int dedisp_plan_launches_per_execute(const dedisp_plan *p) {
     if (!p) return -1;
-    return resolve_kernel(p) == DEDISP_KERNEL_SUBBAND ? (int)p->sb.first_chan.size() - 1 : 1;
+    return subband_launches(p, resolve_kernel(p));
 }
 
 const char *dedisp_error_string(int code) {

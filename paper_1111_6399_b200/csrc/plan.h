@@ -16,22 +16,38 @@ struct TiledGeom {
     int cb = 0;          // channels per pipeline stage
 };
 
-// One pass of the SUBBAND kernel = one sub-band of channels [c_begin, c_end) (subband.h).
+// SUBBAND kernel (subband.cu): exact sub-band re-skewed multi-pass with register-window reuse.
+// Thread tile = SB_D DM rows x SB_K consecutive samples; warp = one DM group (SB_D rows) x 32 lanes;
+// CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
+constexpr int SB_D = 8;
+constexpr int SB_K = 16;
+constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
+constexpr int SB_WARPS = 8;           // DM groups per CTA
+constexpr int SB_ROWS = SB_D * SB_WARPS;
+constexpr int SB_OMAX = 12;           // largest in-window offset a row may have (switch cases 0..SB_OMAX)
+constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel (7)
+constexpr int SB_CB = 8;              // channels per pipeline stage
+constexpr int SB_STAGES = 3;
+constexpr int SB_NCH_MAX = 224;       // staged chunks per channel the slot can hold (logical)
+
+struct SubbandPass {
+    int c_begin = 0, c_end = 0, c_ref = 0;
+    int max_skew = 0;                 // max_d s(c_ref, d)
+};
+
 struct SubbandGeom {
     bool ok = false;
-    int variant = 0;                 // index into the kernel variant table
-    std::vector<int> first_chan;     // G+1 boundaries
-    int ngroups = 0;                 // DM groups of SB_D rows
-    int max_skew = 0;                // max over passes/CTAs of the parallelogram skew (samples)
-    std::vector<uint32_t> win_len;   // per (pass, cta-row-block, channel) staged window length
-    std::vector<uint64_t> records;   // packed per (channel, DM group) records, see subband.h
-    std::vector<int32_t> cta_meta;   // per (channel, cta-row-block): window start rel. to skew origin
+    std::vector<SubbandPass> passes;
+    int ngroups = 0, nblk = 0;
+    // per (channel, group): bits 0..15 chunk base a, bits 16..47 eight 4-bit offsets o_j (subband.cu)
+    std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]
+    // per (channel, block): {window base r (multiple of 4, relative to u), chunks to stage}
+    std::vector<int32_t> meta;        // [nchans][nblk][2]
+    std::vector<int32_t> skew;        // [npasses][ndm] = s(c_ref(pass), d)
     uint64_t *d_records = nullptr;
-    int32_t *d_cta_meta = nullptr;
-    int32_t *d_skew = nullptr;       // per (pass, d): s(c_ref(pass), d)
-    std::vector<int32_t> skew;
-    int slot_words = 0;
-    int cb = 0;
+    int32_t *d_meta = nullptr;
+    int32_t *d_skew = nullptr;
+    int max_nch = 0;                  // largest staged chunk count (sizes the shared-memory slot)
 };
 
 struct dedisp_plan {
@@ -51,6 +67,9 @@ struct dedisp_plan {
     // scratch of dedisp_execute_host (grown on demand, freed at destroy)
     void *d_host_in = nullptr, *d_host_out = nullptr;
     size_t host_in_bytes = 0, host_out_bytes = 0;
+    // fp32 staging copy of the input for the SUBBAND kernel (u8/f16 input, or rows not 16-B aligned)
+    float *d_conv = nullptr;
+    size_t conv_bytes = 0;
 };
 
 inline int dtype_esize(int dtype) { return dtype == DEDISP_U8 ? 1 : dtype == DEDISP_F16 ? 2 : 4; }
@@ -78,7 +97,9 @@ void subband_build(dedisp_plan *p);            // host tables; sets p->sb.ok
 cudaError_t subband_upload(dedisp_plan *p);
 void subband_free(dedisp_plan *p);
 long long subband_verify_records(const dedisp_plan *p);
-cudaError_t launch_subband(const dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,
+int subband_launches(const dedisp_plan *p, int resolved_kernel);  // kernel launches per execute
+cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams);  // staging-copy scratch
+cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,
                            void *d_out, long long out_stride, Batch b, cudaStream_t st);
 
 // plan.cu (shared by the ABI entry points and stream.cu)

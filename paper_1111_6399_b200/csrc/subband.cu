@@ -1,26 +1,487 @@
-// subband.cu — SUBBAND kernel (exact sub-band re-skewed multi-pass with register-window reuse).
+// subband.cu — the SUBBAND kernel: exact sub-band re-skewed multi-pass brute-force de-dispersion
+// with register-window reuse across adjacent DM trials.
 //
-// Not built yet: subband_build() leaves p->sb.ok = false, so AUTO resolves to the TILED kernel and
-// dedisp_plan_set_kernel(DEDISP_KERNEL_SUBBAND) returns DEDISP_EUNSUPPORTED. The entry points exist
-// so that the plan code and the ABI are stable.
+// What it computes is still exactly out[d][t] = sum_c in[c][t + s(c,d)] (§2) with every
+// (c,d) using its own rounded delay s(c,d) from the plan's table — no sub-band approximation.
+//
+// Why: one shared-memory word per add caps a kernel at 32 of the SM's 128 add lanes per clock
+// (measured, profiles/r1_microbench.md). The paper's answer on Fermi — a thread keeps several time
+// samples of one DM in registers and the block's (f,t) lines are reused from L1 —
+// is kept, and extended: a thread owns SB_D adjacent DM trials x SB_K consecutive samples and loads
+// the union of the SB_D windows ONCE into registers, so one loaded word feeds up to SB_D adds.
+// That only pays when adjacent trials' delays differ by a few samples. The survey configs' DM plans
+// are much coarser than the paper's (ndm = nchans), so the channels are split into sub-bands and
+// each sub-band is processed in the skewed time coordinate u = t + s(c_ref, d): the residual delay
+// r(c,d) = s(c,d) - s(c_ref,d) varies by <= SB_OMAX-3 samples across a thread's SB_D rows.
+// One kernel launch per sub-band ("pass"); pass 0 stores, later passes add into out.
+//
+// Per channel a thread: 1 broadcast LDS of its record, SB_WCHUNKS LDS.128 of the window, then for
+// each of its SB_D rows a warp-uniform switch on the row's offset o_j into SB_K adds with static
+// register indices (registers cannot be indexed dynamically).
+#include <algorithm>
+#include <cstring>
+#include <type_traits>
+
 #include "plan.h"
 
-void subband_build(dedisp_plan *p) { p->sb = SubbandGeom(); }
+namespace {
 
-cudaError_t subband_upload(dedisp_plan *) { return cudaSuccess; }
+inline int floor4(int v) { return v & ~3; }  // toward -inf, two's complement
+
+// Residual-delay geometry of channels [cb, ce) against reference channel cr. Returns false if some
+// group's in-window offsets would exceed SB_OMAX or a block's staged window exceeds SB_NCH_MAX.
+// With `emit`, writes records/meta for those channels.
+bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
+    const int ndm = p->ndm, ngroups = p->sb.ngroups, nblk = p->sb.nblk;
+    const int32_t *sref = p->shifts.data() + (size_t)cr * ndm;
+    const int gslots = nblk * SB_WARPS;
+    std::vector<int> gmin(gslots), gmax(gslots);
+    for (int c = cb; c < ce; ++c) {
+        const int32_t *sc = p->shifts.data() + (size_t)c * ndm;
+        for (int q = 0; q < ngroups; ++q) {
+            int mn = INT32_MAX, mx = INT32_MIN;
+            for (int j = 0; j < SB_D; ++j) {
+                const int d = std::min(q * SB_D + j, ndm - 1);
+                const int r = sc[d] - sref[d];
+                mn = std::min(mn, r);
+                mx = std::max(mx, r);
+            }
+            gmin[q] = mn;
+            gmax[q] = mx;
+        }
+        for (int q = ngroups; q < gslots; ++q) { gmin[q] = gmin[ngroups - 1]; gmax[q] = gmax[ngroups - 1]; }
+        for (int b = 0; b < nblk; ++b) {
+            int bmin = INT32_MAX;
+            for (int w = 0; w < SB_WARPS; ++w) bmin = std::min(bmin, gmin[b * SB_WARPS + w]);
+            const int rbase = floor4(bmin);
+            int amax = 0;
+            for (int w = 0; w < SB_WARPS; ++w) {
+                const int q = b * SB_WARPS + w;
+                const int a = (gmin[q] - rbase) >> 2;
+                if (gmax[q] - rbase - 4 * a > SB_OMAX) return false;
+                amax = std::max(amax, a);
+                if (emit) {
+                    uint64_t rec = (uint64_t)a;
+                    const int qq = std::min(q, ngroups - 1);
+                    for (int j = 0; j < SB_D; ++j) {
+                        const int d = std::min(qq * SB_D + j, ndm - 1);
+                        const int o = (sc[d] - sref[d]) - rbase - 4 * a;
+                        rec |= (uint64_t)o << (16 + 4 * j);
+                    }
+                    p->sb.records[(size_t)c * gslots + q] = rec;
+                }
+            }
+            const int nch = amax + 4 * 31 + SB_WCHUNKS;
+            if (nch > SB_NCH_MAX || amax > 0xffff) return false;
+            if (emit) {
+                p->sb.meta[((size_t)c * nblk + b) * 2 + 0] = rbase;
+                p->sb.meta[((size_t)c * nblk + b) * 2 + 1] = nch;
+                p->sb.max_nch = std::max(p->sb.max_nch, nch);
+            }
+        }
+    }
+    return true;
+}
+
+// Reference channel for [cb, ce): the one whose delay at the largest DM is closest to the middle of
+// the sub-band's delay range (delays are proportional to f^-2 - f_top^-2, so this halves |r|).
+int pick_ref(const dedisp_plan *p, int cb, int ce) {
+    const int ndm = p->ndm;
+    auto sl = [&](int c) { return (long long)p->shifts[(size_t)c * ndm + ndm - 1]; };
+    const long long mid2 = sl(cb) + sl(ce - 1);
+    int best = cb;
+    long long bestd = INT64_MAX;
+    int lo = cb, hi = ce - 1;  // sl is non-decreasing in c: binary search for 2*sl(c) >= mid2
+    while (lo < hi) {
+        const int m = (lo + hi) / 2;
+        if (2 * sl(m) >= mid2) hi = m; else lo = m + 1;
+    }
+    for (int c = std::max(cb, lo - 1); c <= std::min(ce - 1, lo + 1); ++c) {
+        const long long dd = std::llabs(2 * sl(c) - mid2);
+        if (dd < bestd) { bestd = dd; best = c; }
+    }
+    return best;
+}
+
+}  // namespace
+
+void subband_build(dedisp_plan *p) {
+    p->sb = SubbandGeom();
+    SubbandGeom &sb = p->sb;
+    const int nchans = p->nchans, ndm = p->ndm;
+    sb.ngroups = (ndm + SB_D - 1) / SB_D;
+    sb.nblk = (sb.ngroups + SB_WARPS - 1) / SB_WARPS;
+    const size_t gslots = (size_t)sb.nblk * SB_WARPS;
+    if ((double)nchans * gslots * 8.0 > 4.0e9) return;  // record table would not fit sensibly
+    if (p->dtype == DEDISP_U8 && (double)nchans * 255.0 >= 16777216.0) return;  // fp32 sums must stay exact
+    // greedy: extend each sub-band as far as the geometry admits (exponential then binary search)
+    int cb = 0;
+    while (cb < nchans) {
+        auto ok = [&](int ce) { return pass_geometry(p, cb, ce, pick_ref(p, cb, ce), false); };
+        if (!ok(cb + 1)) return;  // a single channel against itself always has r = 0; defensive
+        int good = cb + 1, step = 1;
+        while (good < nchans) {
+            const int trial = std::min(nchans, good + step);
+            if (ok(trial)) { good = trial; step *= 2; } else break;
+        }
+        int bad = std::min(nchans, good + step);  // first known-bad (or nchans if all good)
+        if (good < nchans) {
+            int lo = good, hi = bad;  // ok(lo) true, ok(hi) false
+            while (hi - lo > 1) {
+                const int m = (lo + hi) / 2;
+                if (ok(m)) lo = m; else hi = m;
+            }
+            good = lo;
+        }
+        SubbandPass ps;
+        ps.c_begin = cb;
+        ps.c_end = good;
+        ps.c_ref = pick_ref(p, cb, good);
+        sb.passes.push_back(ps);
+        cb = good;
+        if (sb.passes.size() > 512) { sb.passes.clear(); return; }  // hopelessly coarse plan: use TILED
+    }
+    sb.records.assign((size_t)nchans * gslots, 0);
+    sb.meta.assign((size_t)nchans * sb.nblk * 2, 0);
+    sb.skew.assign(sb.passes.size() * (size_t)ndm, 0);
+    for (size_t g = 0; g < sb.passes.size(); ++g) {
+        SubbandPass &ps = sb.passes[g];
+        if (!pass_geometry(p, ps.c_begin, ps.c_end, ps.c_ref, true)) { sb = SubbandGeom(); return; }
+        const int32_t *sref = p->shifts.data() + (size_t)ps.c_ref * ndm;
+        std::memcpy(sb.skew.data() + g * (size_t)ndm, sref, (size_t)ndm * sizeof(int32_t));
+        ps.max_skew = sref[ndm - 1];
+    }
+    sb.ok = true;
+}
+
+// Rebuild s(c,d) from the packed records (+ meta + skew) and compare with the table: the records
+// are all the kernel sees, so 0 mismatches means the kernel's address arithmetic encodes exactly
+// the plan's delays.
+long long subband_verify_records(const dedisp_plan *p) {
+    const SubbandGeom &sb = p->sb;
+    if (!sb.ok) return -1;
+    const int ndm = p->ndm;
+    const size_t gslots = (size_t)sb.nblk * SB_WARPS;
+    long long bad = 0;
+    std::vector<char> seen(p->nchans, 0);
+    for (size_t g = 0; g < sb.passes.size(); ++g) {
+        const SubbandPass &ps = sb.passes[g];
+        for (int c = ps.c_begin; c < ps.c_end; ++c) {
+            seen[c]++;
+            for (int d = 0; d < ndm; ++d) {
+                const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
+                const uint64_t rec = sb.records[(size_t)c * gslots + q];
+                const int a = (int)(rec & 0xffff), o = (int)((rec >> (16 + 4 * j)) & 15);
+                const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
+                const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
+                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 4 * a + o;
+                if (s != p->shifts[(size_t)c * ndm + d] || a + 4 * 31 + SB_WCHUNKS > nch || (rbase & 3)) ++bad;
+            }
+        }
+    }
+    for (int c = 0; c < p->nchans; ++c) bad += seen[c] != 1;
+    return bad;
+}
+
+// =====================================================================================
+// device side
+// =====================================================================================
+#include <cuda_fp16.h>
+
+namespace {
+
+constexpr int SB_THREADS = SB_WARPS * 32;
+
+__host__ __device__ constexpr int sb_phys(int chunk) { return chunk + (chunk >> 2); }  // 1 pad chunk per 4
+constexpr int SB_SLOT_CHUNKS_MAX = sb_phys(SB_NCH_MAX) + 1;
+
+__device__ __forceinline__ void sb_cp_async16(void *smem, const void *gmem, int src_bytes) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void sb_cp_async8(void *smem, const void *gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void sb_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void sb_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+struct SbArgs {
+    const float *in;          // fp32 input, 16-byte aligned, stride % 4 == 0
+    long long in_stride;      // elements
+    long long in_total;       // readable elements per beam starting at `in`
+    long long in_beam;        // elements between beams
+    void *out;
+    long long out_stride, out_beam;
+    long long nsamp_out;
+    const uint64_t *records;  // [nchans][gslots]
+    const int32_t *meta;      // [nchans][nblk][2]
+    const int32_t *skew;      // this pass: [ndm]
+    int c_begin, c_end;
+    int ndm, nblk, gslots;
+    int slot_chunks;          // physical 16-byte chunks per staged channel
+    int first;                // 1: store, 0: add into out
+};
+
+// window load: SB_WCHUNKS aligned 16-byte chunks starting at logical chunk a + 4*lane; the padded
+// layout makes the physical step irregular only through (a & 3), which is warp-uniform -> AR.
+template <int AR>
+__device__ __forceinline__ void sb_load_window(const float4 *base, float (&w)[4 * SB_WCHUNKS]) {
+#pragma unroll
+    for (int m = 0; m < SB_WCHUNKS; ++m) {
+        const float4 v = base[m + ((AR + m) >> 2)];
+        w[4 * m + 0] = v.x; w[4 * m + 1] = v.y; w[4 * m + 2] = v.z; w[4 * m + 3] = v.w;
+    }
+}
+
+template <int O>
+__device__ __forceinline__ void sb_add_row(float (&acc)[SB_K], const float (&w)[4 * SB_WCHUNKS]) {
+#pragma unroll
+    for (int k = 0; k < SB_K; ++k) acc[k] += w[O + k];
+}
+
+__device__ __forceinline__ void sb_dispatch_row(int o, float (&acc)[SB_K], const float (&w)[4 * SB_WCHUNKS]) {
+    switch (o) {
+        case 0: sb_add_row<0>(acc, w); break;
+        case 1: sb_add_row<1>(acc, w); break;
+        case 2: sb_add_row<2>(acc, w); break;
+        case 3: sb_add_row<3>(acc, w); break;
+        case 4: sb_add_row<4>(acc, w); break;
+        case 5: sb_add_row<5>(acc, w); break;
+        case 6: sb_add_row<6>(acc, w); break;
+        case 7: sb_add_row<7>(acc, w); break;
+        case 8: sb_add_row<8>(acc, w); break;
+        case 9: sb_add_row<9>(acc, w); break;
+        case 10: sb_add_row<10>(acc, w); break;
+        case 11: sb_add_row<11>(acc, w); break;
+        default: sb_add_row<12>(acc, w); break;
+    }
+}
+
+template <typename OutT>
+__global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
+    extern __shared__ __align__(16) unsigned char sb_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int blk = blockIdx.x % A.nblk;
+    const long long U0 = (long long)(blockIdx.x / A.nblk) * SB_T;
+    const int d_first = blk * SB_ROWS;
+    const int d_last = min(A.ndm, d_first + SB_ROWS) - 1;
+    // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
+    if (U0 + SB_T <= (long long)__ldg(A.skew + d_first) || U0 >= (long long)__ldg(A.skew + d_last) + A.nsamp_out) return;
+
+    const float *in = A.in + (size_t)blockIdx.z * A.in_beam;
+    const size_t slot_bytes = (size_t)A.slot_chunks * 16;
+    const size_t stage_bytes = SB_CB * slot_bytes;
+    unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
+    uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
+
+    float acc[SB_D][SB_K];
+#pragma unroll
+    for (int j = 0; j < SB_D; ++j)
+#pragma unroll
+        for (int k = 0; k < SB_K; ++k) acc[j][k] = 0.f;
+
+    const int nchan = A.c_end - A.c_begin;
+    const int nstages = (nchan + SB_CB - 1) / SB_CB;
+
+    auto issue = [&](int stage) {
+        if (stage < nstages) {
+            const int buf = stage % SB_STAGES;
+            for (int ch = 0; ch < SB_CB; ++ch) {
+                const int c = A.c_begin + stage * SB_CB + ch;
+                if (c >= A.c_end) break;
+                const int2 mt = __ldg(reinterpret_cast<const int2 *>(A.meta) + (size_t)c * A.nblk + blk);
+                const long long e0 = (long long)c * A.in_stride + U0 + mt.x;
+                unsigned char *slot = sdata + buf * stage_bytes + ch * slot_bytes;
+                for (int i = tid; i < mt.y; i += SB_THREADS) {
+                    const long long e = e0 + 4 * (long long)i;
+                    long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
+                    valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
+                    sb_cp_async16(slot + sb_phys(i) * 16, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
+                }
+            }
+            if (tid < SB_CB * SB_WARPS) {
+                const int ch = tid / SB_WARPS, w = tid % SB_WARPS;
+                const int c = A.c_begin + stage * SB_CB + ch;
+                if (c < A.c_end)
+                    sb_cp_async8(srec + (buf * SB_CB + ch) * SB_WARPS + w, A.records + (size_t)c * A.gslots + blk * SB_WARPS + w);
+            }
+        }
+        sb_commit();
+    };
+
+    issue(0);
+    issue(1);
+    for (int stage = 0; stage < nstages; ++stage) {
+        issue(stage + 2);
+        sb_wait<2>();
+        __syncthreads();
+        const int buf = stage % SB_STAGES;
+        const int nch = min(SB_CB, nchan - stage * SB_CB);
+        for (int ch = 0; ch < nch; ++ch) {
+            const uint2 rec = srec[(buf * SB_CB + ch) * SB_WARPS + warp];
+            const int a = rec.x & 0xffff;
+            const unsigned obits = (rec.x >> 16) | (rec.y << 16);
+            const float4 *base = reinterpret_cast<const float4 *>(sdata + buf * stage_bytes + ch * slot_bytes) +
+                                 5 * lane + a + (a >> 2);
+            float w[4 * SB_WCHUNKS];
+            switch (a & 3) {
+                case 0: sb_load_window<0>(base, w); break;
+                case 1: sb_load_window<1>(base, w); break;
+                case 2: sb_load_window<2>(base, w); break;
+                default: sb_load_window<3>(base, w); break;
+            }
+#pragma unroll
+            for (int j = 0; j < SB_D; ++j) sb_dispatch_row((obits >> (4 * j)) & 15, acc[j], w);
+        }
+        __syncthreads();
+    }
+
+    OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
+#pragma unroll
+    for (int j = 0; j < SB_D; ++j) {
+        const int d = d_first + warp * SB_D + j;
+        if (d >= A.ndm) continue;
+        const long long t0 = U0 + SB_K * lane - (long long)__ldg(A.skew + d);
+        OutT *orow = out + (size_t)d * A.out_stride;
+#pragma unroll
+        for (int k = 0; k < SB_K; ++k) {
+            const long long t = t0 + k;
+            if (t >= 0 && t < A.nsamp_out) {
+                if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
+                    const int v = __float2int_rn(acc[j][k]);
+                    orow[t] = A.first ? v : orow[t] + v;
+                } else {
+                    orow[t] = A.first ? acc[j][k] : orow[t] + acc[j][k];
+                }
+            }
+        }
+    }
+}
+
+// input staging copy: any dtype / any stride -> fp32 rows with a 16-byte-aligned pitch
+template <typename TIN>
+__global__ void __launch_bounds__(256) dedisp_to_f32_kernel(const TIN *__restrict__ in, long long in_stride, long long in_beam,
+                                                            float *__restrict__ out, long long out_stride, long long out_beam,
+                                                            long long ncols) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ncols) return;
+    const TIN *src = in + (size_t)blockIdx.z * in_beam + (size_t)blockIdx.y * in_stride;
+    float *dst = out + (size_t)blockIdx.z * out_beam + (size_t)blockIdx.y * out_stride;
+    float v;
+    if constexpr (std::is_same<TIN, __half>::value) v = __half2float(src[i]);
+    else v = (float)src[i];
+    dst[i] = v;
+}
+
+}  // namespace
+
+// =====================================================================================
+// host launch
+// =====================================================================================
+cudaError_t subband_upload(dedisp_plan *p) {
+    SubbandGeom &sb = p->sb;
+    if (!sb.ok) return cudaSuccess;
+    cudaError_t e = cudaMalloc(&sb.d_records, sb.records.size() * sizeof(uint64_t));
+    if (e == cudaSuccess) e = cudaMemcpy(sb.d_records, sb.records.data(), sb.records.size() * sizeof(uint64_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&sb.d_meta, sb.meta.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemcpy(sb.d_meta, sb.meta.data(), sb.meta.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&sb.d_skew, sb.skew.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemcpy(sb.d_skew, sb.skew.data(), sb.skew.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    return e;
+}
 
 void subband_free(dedisp_plan *p) {
     if (p->sb.d_records) cudaFree(p->sb.d_records);
-    if (p->sb.d_cta_meta) cudaFree(p->sb.d_cta_meta);
+    if (p->sb.d_meta) cudaFree(p->sb.d_meta);
     if (p->sb.d_skew) cudaFree(p->sb.d_skew);
+    if (p->d_conv) cudaFree(p->d_conv);
     p->sb.d_records = nullptr;
-    p->sb.d_cta_meta = nullptr;
+    p->sb.d_meta = nullptr;
     p->sb.d_skew = nullptr;
+    p->d_conv = nullptr;
+    p->conv_bytes = 0;
 }
 
-long long subband_verify_records(const dedisp_plan *) { return -1; }
+static bool sb_needs_staging_copy(const dedisp_plan *p, const void *d_in, long long in_stride, Batch b) {
+    return p->dtype != DEDISP_F32 || ((uintptr_t)d_in & 15) != 0 || (in_stride & 3) != 0 || (b.n > 1 && (b.in_stride & 3) != 0);
+}
 
-cudaError_t launch_subband(const dedisp_plan *, const void *, long long, long long, void *, long long, Batch,
-                           cudaStream_t) {
-    return cudaErrorNotSupported;
+int subband_launches(const dedisp_plan *p, int resolved_kernel) {
+    if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
+    return (int)p->sb.passes.size() + (p->dtype != DEDISP_F32 ? 1 : 0);
+}
+
+cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams) {
+    const long long pitch = (nsamp_out + p->maxshift + 3) & ~3ll;
+    const size_t need = (size_t)nbeams * p->nchans * pitch * sizeof(float);
+    if (need <= p->conv_bytes) return cudaSuccess;
+    if (p->d_conv) cudaFree(p->d_conv);
+    p->d_conv = nullptr;
+    p->conv_bytes = 0;
+    cudaError_t e = cudaMalloc(&p->d_conv, need);
+    if (e == cudaSuccess) p->conv_bytes = need;
+    return e;
+}
+
+cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
+                           long long out_stride, Batch b, cudaStream_t st) {
+    const SubbandGeom &sb = p->sb;
+    const long long nsamp_in = nsamp_out + p->maxshift;
+    SbArgs A;
+    A.in = (const float *)d_in;
+    A.in_stride = in_stride;
+    A.in_total = (long long)(p->nchans - 1) * in_stride + nsamp_in;
+    A.in_beam = b.in_stride;
+    if (sb_needs_staging_copy(p, d_in, in_stride, b)) {
+        const long long pitch = (nsamp_in + 3) & ~3ll;
+        cudaError_t e = subband_reserve(p, nsamp_out, b.n);
+        if (e != cudaSuccess) return e;
+        dim3 grid((unsigned)((nsamp_in + 255) / 256), (unsigned)p->nchans, (unsigned)b.n);
+        const long long obeam = (long long)p->nchans * pitch;
+        switch (p->dtype) {
+            case DEDISP_U8:
+                dedisp_to_f32_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                break;
+            case DEDISP_F16:
+                dedisp_to_f32_kernel<__half><<<grid, 256, 0, st>>>((const __half *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                break;
+            default:
+                dedisp_to_f32_kernel<float><<<grid, 256, 0, st>>>((const float *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                break;
+        }
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        A.in = p->d_conv;
+        A.in_stride = pitch;
+        A.in_total = obeam;
+        A.in_beam = obeam;
+    }
+    A.out = d_out;
+    A.out_stride = out_stride;
+    A.out_beam = b.out_stride;
+    A.nsamp_out = nsamp_out;
+    A.records = sb.d_records;
+    A.meta = sb.d_meta;
+    A.ndm = p->ndm;
+    A.nblk = sb.nblk;
+    A.gslots = sb.nblk * SB_WARPS;
+    A.slot_chunks = sb_phys(sb.max_nch) + 1;
+    const size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8;
+    auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    for (size_t g = 0; g < sb.passes.size(); ++g) {
+        const SubbandPass &ps = sb.passes[g];
+        A.skew = sb.d_skew + g * (size_t)p->ndm;
+        A.c_begin = ps.c_begin;
+        A.c_end = ps.c_end;
+        A.first = g == 0;
+        const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
+        dim3 grid((unsigned)(ntiles * sb.nblk), 1, (unsigned)b.n);
+        kern<<<grid, SB_THREADS, smem, st>>>(A);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }

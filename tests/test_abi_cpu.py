@@ -85,3 +85,16 @@ def test_no_gpu_means_loud_failure():
         pytest.skip("GPU present")
     with pytest.raises(P.DedispError):
         P.Plan.from_config(CONFIGS["c1"])
+
+
+@pytest.mark.parametrize("name", list(CONFIGS))
+def test_subband_records_encode_exactly_the_shift_table(name):
+    """The SUBBAND kernel only ever sees packed records (+ window bases + per-pass skews); rebuilding
+    s(c,d) from them on the host must give back the plan's table, and every channel must belong to
+    exactly one pass (dedisp_plan_verify_records == 0 mismatches)."""
+    plan = P.Plan.from_config(CONFIGS[name], host_only=True)
+    g = plan.num_subbands()
+    assert g >= 1
+    sb = plan.subbands()
+    assert sb[0] == 0 and sb[-1] == CONFIGS[name].nchans and np.all(np.diff(sb) > 0)
+    assert plan.verify_records() == 0
