@@ -39,7 +39,7 @@ struct SubbandGeom {
     bool ok = false;
     std::vector<SubbandPass> passes;
     int ngroups = 0, nblk = 0;
-    // per (channel, group): bits 0..15 chunk base a, bits 16..47 eight 4-bit offsets o_j (subband.cu)
+    // per (channel, group): bits 0..31 eight 4-bit offsets o_j, bits 32..47 chunk base a (subband.cu)
     std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]
     // per (channel, block): {window base r (multiple of 4, relative to u), chunks to stage}
     std::vector<int32_t> meta;        // [nchans][nblk][2]

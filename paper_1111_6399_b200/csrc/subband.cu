@@ -16,8 +16,9 @@
 // One kernel launch per sub-band ("pass"); pass 0 stores, later passes add into out.
 //
 // Per channel a thread: 1 broadcast LDS of its record, SB_WCHUNKS LDS.128 of the window, then for
-// each of its SB_D rows a warp-uniform switch on the row's offset o_j into SB_K adds with static
-// register indices (registers cannot be indexed dynamically).
+// each of its SB_D rows a warp-uniform jump on the row's offset o_j into SB_K/2 FADD2 with static
+// register operands (registers cannot be indexed dynamically). That body is generated inline PTX:
+// see gen_subband_rows.py for why and subband_rows.inc for the text.
 #include <algorithm>
 #include <cstring>
 #include <type_traits>
@@ -61,12 +62,12 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
                 if (gmax[q] - rbase - 4 * a > SB_OMAX) return false;
                 amax = std::max(amax, a);
                 if (emit) {
-                    uint64_t rec = (uint64_t)a;
+                    uint64_t rec = (uint64_t)a << 32;
                     const int qq = std::min(q, ngroups - 1);
                     for (int j = 0; j < SB_D; ++j) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
                         const int o = (sc[d] - sref[d]) - rbase - 4 * a;
-                        rec |= (uint64_t)o << (16 + 4 * j);
+                        rec |= (uint64_t)o << (4 * j);
                     }
                     p->sb.records[(size_t)c * gslots + q] = rec;
                 }
@@ -171,7 +172,7 @@ long long subband_verify_records(const dedisp_plan *p) {
             for (int d = 0; d < ndm; ++d) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
                 const uint64_t rec = sb.records[(size_t)c * gslots + q];
-                const int a = (int)(rec & 0xffff), o = (int)((rec >> (16 + 4 * j)) & 15);
+                const int a = (int)((rec >> 32) & 0xffff), o = (int)((rec >> (4 * j)) & 15);
                 const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
                 const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
                 const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 4 * a + o;
@@ -191,17 +192,17 @@ long long subband_verify_records(const dedisp_plan *p) {
 namespace {
 
 constexpr int SB_THREADS = SB_WARPS * 32;
+static_assert(SB_CB == SB_WARPS, "staging maps one warp to one channel of a stage");
+static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
 __host__ __device__ constexpr int sb_phys(int chunk) { return chunk + (chunk >> 2); }  // 1 pad chunk per 4
 constexpr int SB_SLOT_CHUNKS_MAX = sb_phys(SB_NCH_MAX) + 1;
 
-__device__ __forceinline__ void sb_cp_async16(void *smem, const void *gmem, int src_bytes) {
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
+__device__ __forceinline__ void sb_cp_async16_s(unsigned sa, const void *gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
 }
-__device__ __forceinline__ void sb_cp_async8(void *smem, const void *gmem) {
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem));
+__device__ __forceinline__ void sb_cp_async16_zs(unsigned sa, const void *gmem, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
 }
 __device__ __forceinline__ void sb_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void sb_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
@@ -221,42 +222,10 @@ struct SbArgs {
     int ndm, nblk, gslots;
     int slot_chunks;          // physical 16-byte chunks per staged channel
     int first;                // 1: store, 0: add into out
+    unsigned zero;            // always 0, opaque to the compiler (subband_rows.inc)
 };
 
-// window load: SB_WCHUNKS aligned 16-byte chunks starting at logical chunk a + 4*lane; the padded
-// layout makes the physical step irregular only through (a & 3), which is warp-uniform -> AR.
-template <int AR>
-__device__ __forceinline__ void sb_load_window(const float4 *base, float (&w)[4 * SB_WCHUNKS]) {
-#pragma unroll
-    for (int m = 0; m < SB_WCHUNKS; ++m) {
-        const float4 v = base[m + ((AR + m) >> 2)];
-        w[4 * m + 0] = v.x; w[4 * m + 1] = v.y; w[4 * m + 2] = v.z; w[4 * m + 3] = v.w;
-    }
-}
-
-template <int O>
-__device__ __forceinline__ void sb_add_row(float (&acc)[SB_K], const float (&w)[4 * SB_WCHUNKS]) {
-#pragma unroll
-    for (int k = 0; k < SB_K; ++k) acc[k] += w[O + k];
-}
-
-__device__ __forceinline__ void sb_dispatch_row(int o, float (&acc)[SB_K], const float (&w)[4 * SB_WCHUNKS]) {
-    switch (o) {
-        case 0: sb_add_row<0>(acc, w); break;
-        case 1: sb_add_row<1>(acc, w); break;
-        case 2: sb_add_row<2>(acc, w); break;
-        case 3: sb_add_row<3>(acc, w); break;
-        case 4: sb_add_row<4>(acc, w); break;
-        case 5: sb_add_row<5>(acc, w); break;
-        case 6: sb_add_row<6>(acc, w); break;
-        case 7: sb_add_row<7>(acc, w); break;
-        case 8: sb_add_row<8>(acc, w); break;
-        case 9: sb_add_row<9>(acc, w); break;
-        case 10: sb_add_row<10>(acc, w); break;
-        case 11: sb_add_row<11>(acc, w); break;
-        default: sb_add_row<12>(acc, w); break;
-    }
-}
+typedef unsigned long long sb_u64;  // one aligned register pair = two fp32 accumulators (FADD2 operand)
 
 template <typename OutT>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
@@ -270,42 +239,52 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     if (U0 + SB_T <= (long long)__ldg(A.skew + d_first) || U0 >= (long long)__ldg(A.skew + d_last) + A.nsamp_out) return;
 
     const float *in = A.in + (size_t)blockIdx.z * A.in_beam;
-    const size_t slot_bytes = (size_t)A.slot_chunks * 16;
-    const size_t stage_bytes = SB_CB * slot_bytes;
+    const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
+    const unsigned stage_bytes = SB_CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
     uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
+    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 80u * lane;  // 5 chunks per lane (sb_phys)
+    const unsigned zero = A.zero;
 
-    float acc[SB_D][SB_K];
+    sb_u64 acc[SB_D][SB_K / 2];
 #pragma unroll
     for (int j = 0; j < SB_D; ++j)
 #pragma unroll
-        for (int k = 0; k < SB_K; ++k) acc[j][k] = 0.f;
+        for (int k = 0; k < SB_K / 2; ++k) acc[j][k] = 0ull;
 
     const int nchan = A.c_end - A.c_begin;
     const int nstages = (nchan + SB_CB - 1) / SB_CB;
 
+    // Staging: warp w copies channel w of the stage (SB_CB == SB_WARPS); lane l copies logical chunks
+    // l, l+32, ... into the padded layout (sb_phys(l + 32 it) = sb_phys(l) + 40 it). All of a warp's
+    // quantities but the lane term are warp-uniform; only windows that cross either end of the input
+    // allocation take the bounds-checked zero-filling path.
+    const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sdata);
+    const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
     auto issue = [&](int stage) {
-        if (stage < nstages) {
+        const int c = A.c_begin + stage * SB_CB + warp;
+        if (stage < nstages && c < A.c_end) {
             const int buf = stage % SB_STAGES;
-            for (int ch = 0; ch < SB_CB; ++ch) {
-                const int c = A.c_begin + stage * SB_CB + ch;
-                if (c >= A.c_end) break;
-                const int2 mt = __ldg(reinterpret_cast<const int2 *>(A.meta) + (size_t)c * A.nblk + blk);
-                const long long e0 = (long long)c * A.in_stride + U0 + mt.x;
-                unsigned char *slot = sdata + buf * stage_bytes + ch * slot_bytes;
-                for (int i = tid; i < mt.y; i += SB_THREADS) {
-                    const long long e = e0 + 4 * (long long)i;
+            const int2 mt = __ldg(meta2 + (size_t)c * A.nblk + blk);
+            const long long e0 = (long long)c * A.in_stride + U0 + mt.x;
+            const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * (lane + (lane >> 2));
+            const float *src = in + e0 + 4 * lane;
+            if (e0 >= 0 && e0 + 4ll * mt.y <= A.in_total) {
+#pragma unroll
+                for (int it = 0; it < SB_NCH_MAX / 32; ++it)
+                    if (lane + 32 * it < mt.y) sb_cp_async16_s(dst + 640u * it, src + 128 * it);
+            } else {
+                for (int it = 0; it < SB_NCH_MAX / 32; ++it) {
+                    if (lane + 32 * it >= mt.y) break;
+                    const long long e = e0 + 4 * lane + 128ll * it;
                     long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
                     valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
-                    sb_cp_async16(slot + sb_phys(i) * 16, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
+                    sb_cp_async16_zs(dst + 640u * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
                 }
             }
-            if (tid < SB_CB * SB_WARPS) {
-                const int ch = tid / SB_WARPS, w = tid % SB_WARPS;
-                const int c = A.c_begin + stage * SB_CB + ch;
-                if (c < A.c_end)
-                    sb_cp_async8(srec + (buf * SB_CB + ch) * SB_WARPS + w, A.records + (size_t)c * A.gslots + blk * SB_WARPS + w);
-            }
+            if (lane < 4)   // the 8 warps' records of this channel: 64 contiguous bytes
+                sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * SB_CB + warp) * SB_WARPS) + 16u * lane,
+                                reinterpret_cast<const char *>(A.records + (size_t)c * A.gslots + blk * SB_WARPS) + 16 * lane);
         }
         sb_commit();
     };
@@ -318,21 +297,15 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         __syncthreads();
         const int buf = stage % SB_STAGES;
         const int nch = min(SB_CB, nchan - stage * SB_CB);
-        for (int ch = 0; ch < nch; ++ch) {
-            const uint2 rec = srec[(buf * SB_CB + ch) * SB_WARPS + warp];
-            const int a = rec.x & 0xffff;
-            const unsigned obits = (rec.x >> 16) | (rec.y << 16);
-            const float4 *base = reinterpret_cast<const float4 *>(sdata + buf * stage_bytes + ch * slot_bytes) +
-                                 5 * lane + a + (a >> 2);
-            float w[4 * SB_WCHUNKS];
-            switch (a & 3) {
-                case 0: sb_load_window<0>(base, w); break;
-                case 1: sb_load_window<1>(base, w); break;
-                case 2: sb_load_window<2>(base, w); break;
-                default: sb_load_window<3>(base, w); break;
-            }
-#pragma unroll
-            for (int j = 0; j < SB_D; ++j) sb_dispatch_row((obits >> (4 * j)) & 15, acc[j], w);
+        const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
+        unsigned slot_u32 = sdata_u32 + buf * stage_bytes;
+#pragma unroll 1
+        for (int ch = 0; ch < nch; ++ch, recp += SB_WARPS, slot_u32 += slot_bytes) {
+            const uint2 rec = *recp;                       // warp-uniform: x = eight 4-bit o_j, y = chunk base a
+            const unsigned obits = rec.x;
+            const unsigned ar = rec.y & 3u;
+            const unsigned sa = slot_u32 + ((rec.y + (rec.y >> 2)) << 4);
+#include "subband_rows.inc"
         }
         __syncthreads();
     }
@@ -347,12 +320,14 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 #pragma unroll
         for (int k = 0; k < SB_K; ++k) {
             const long long t = t0 + k;
+            const unsigned bits = (k & 1) ? (unsigned)(acc[j][k >> 1] >> 32) : (unsigned)acc[j][k >> 1];
+            const float v = __uint_as_float(bits);
             if (t >= 0 && t < A.nsamp_out) {
                 if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
-                    const int v = __float2int_rn(acc[j][k]);
-                    orow[t] = A.first ? v : orow[t] + v;
+                    const int vi = __float2int_rn(v);
+                    orow[t] = A.first ? vi : orow[t] + vi;
                 } else {
-                    orow[t] = A.first ? acc[j][k] : orow[t] + acc[j][k];
+                    orow[t] = A.first ? v : orow[t] + v;
                 }
             }
         }
@@ -467,6 +442,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.nblk = sb.nblk;
     A.gslots = sb.nblk * SB_WARPS;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
+    A.zero = 0;
     const size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8;
     auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
