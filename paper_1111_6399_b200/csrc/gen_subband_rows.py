@@ -1,85 +1,147 @@
 #!/usr/bin/env python
 """Generates ``subband_rows.inc`` — the per-channel body of the SUBBAND kernel (subband.cu) as one
-inline-PTX statement.  Run ``python gen_subband_rows.py`` after changing a constant; the generated
-file is committed so that the build needs nvcc only.
+inline-PTX statement.  ``python gen_subband_rows.py [D K OMAX [shifted_copy]]`` after changing a
+tile constant; the generated file is committed so that the build needs nvcc only, and subband.cu
+static_asserts that its constants (plan.h) match the ones the file was generated for.
 
-Why PTX: a thread owns SB_D = 8 DM rows x SB_K = 16 consecutive samples and holds the union of its
-rows' input windows in registers; row j needs window words [o_j, o_j + 16) with o_j in 0..SB_OMAX
-known only at run time (warp-uniform).  Registers cannot be indexed dynamically, so each row jumps
-to one of 13 bodies with static register operands.  Written as a C++ ``switch`` nvcc if-converts
+Why PTX: a thread owns SB_D DM rows x SB_K consecutive samples and holds the union of its rows'
+input windows in registers; row j needs window words [o_j, o_j + SB_K) with o_j in 0..SB_OMAX known
+only at run time (warp-uniform).  Registers cannot be indexed dynamically, so each row jumps to one
+of SB_OMAX+1 bodies with static register operands.  Written as a C++ ``switch`` nvcc if-converts
 the bodies into select chains (13 predicated moves per add: measured 9.5 % of the add peak,
-profiles/r1_subband_v1.md); written here as *threaded code* every body ends with the ``brx.idx``
-of the NEXT row, which ptxas lowers to LDC (jump table) + BRX and schedules in the shadow of the
-body's adds.
+profiles/r1_subband.md); written here as *threaded code* every body ends with the ``brx.idx`` of
+the NEXT row, which ptxas lowers to LDC (jump table) + BRX; the table indices of all rows are
+extracted when the channel starts so that the LDC can issue at the top of the previous body.
 
-Adds are ``add.rn.f32x2`` (SASS FADD2: two fp32 adds per lane per issue slot, the only way to
+Adds are ``add.rn.f32x2`` (SASS FADD2: two fp32 adds per lane per issue slot — the only way to
 leave issue slots for anything else at 128 lane-adds/clk/SM).  FADD2 needs its operands in aligned
-64-bit register pairs: even o_j use the window pairs as loaded (w), odd o_j use a copy shifted by
-one word (v), built once per channel with 26 ``or.b32 x, y, zero`` (ALU pipe; ``zero`` is a run-time
-0 so that ptxas cannot turn them into moves and sink 16 of them into every odd body).
+64-bit register pairs: even o_j use the window pairs as loaded (w), odd o_j use pairs shifted by
+one word (v).  With shifted_copy=1 the v pairs are built once per channel with ``or.b32 x, y, zero``
+(ALU pipe; ``zero`` is a run-time 0 so that ptxas cannot turn them into moves and sink them into
+every odd body); with shifted_copy=0 they are plain moves and ptxas sinks 2 moves per FADD2 into
+the odd bodies (fewer registers, more issue slots).
 
-Operands of the statement:  %0..%63  acc[j][k2] (b64, "+l"), then sa (u32 shared address of the
-lane's first window chunk, already including the padded-layout term), ar (= a & 3: which of the
-four pad phases the window starts in), obits (eight 4-bit o_j), zero.
+Operands of the statement:  %0.. acc[j][k2] (b64, "+l"), then sa (u32 shared address of the
+lane's first window chunk, already including the padded-layout term), ar (= a mod SB_K/4: which pad
+phase the window starts in), obits (SB_D 4-bit o_j), zero.
 """
 import os
-
-SB_D, SB_K, SB_OMAX = 8, 16, 12
-K2 = SB_K // 2
-NCHUNK = (SB_K + SB_OMAX + 3) // 4          # 7 16-byte chunks
-NW = 2 * NCHUNK                             # 14 aligned pairs
-NV = NW - 1                                 # 13 shifted pairs
-NO = SB_OMAX + 1
+import sys
 
 
-def acc(j, k):
-    return "%%%d" % (j * K2 + k)
+def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
+    K2 = K // 2
+    P = K // 4                                  # chunks per lane = pad period (one pad chunk per P)
+    NCHUNK = (K + OMAX + 3) // 4
+    NW, NV, NO = 2 * NCHUNK, 2 * NCHUNK - 1, OMAX + 1
+    assert D * 4 <= 32 and OMAX <= 15 and P % 2 == 0
 
+    def acc(j, k):
+        return "%%%d" % (j * K2 + k)
 
-SA, AR, OB, ZERO = ("%%%d" % (SB_D * K2 + i) for i in range(4))
+    SA, AR, OB, ZERO = ("%%%d" % (D * K2 + i) for i in range(4))
+    L = ["{", ".reg .b32 t<%d>, tt;" % D, ".reg .pred q<4>;", ".reg .b64 w<%d>, v<%d>;" % (NW, NV),
+         ".reg .b32 l<%d>, h<%d>, x<%d>, y<%d>;" % (NW, NW, NV, NV)]
+    if head == "brx":
+        L.append("TA: .branchtargets %s;" % ", ".join("LA%d" % r for r in range(P)))
+    if dispatch == "brx":
+        for j in range(D):
+            L.append("T%d: .branchtargets %s;" % (j, ", ".join("R%d_%d" % (j, v) for v in range(NO))))
 
+    def preds(j):
+        # predicates q0..q3 = the four bits of o_j (tree dispatch); set one body ahead of their use
+        out = []
+        for b in range(4):
+            if (1 << b) <= OMAX:
+                out += ["and.b32 tt, %s, %d;" % (OB, 1 << (4 * j + b)), "setp.ne.u32 q%d, tt, 0;" % b]
+        return out
 
-def dispatch(j):
-    return ["bfe.u32 t, %s, %d, 4;" % (OB, 4 * j), "brx.idx.uni t, T%d;" % j]
+    def goto_row(j):
+        if j >= D:
+            return ["bra.uni DONE;"]
+        return ["brx.idx.uni t%d, T%d;" % (j, j)] if dispatch == "brx" else ["bra.uni TREE%d;" % j]
 
+    def body(j, o):
+        out = ["R%d_%d:" % (j, o)]
+        if dispatch == "tree" and j + 1 < D:
+            out += preds(j + 1)
+        for k in range(K2):
+            src = ("v%d" if o & 1 else "w%d") % ((o >> 1) + k)
+            out.append("add.rn.f32x2 %s, %s, %s;" % (acc(j, k), acc(j, k), src))
+        return out + goto_row(j + 1)
 
-def generate():
-    L = ["{", ".reg .b32 t;", ".reg .b64 w<%d>, v<%d>;" % (NW, NV), ".reg .b32 l<%d>, h<%d>, x<%d>, y<%d>;" % (NW, NW, NV, NV)]
-    L.append("TA: .branchtargets %s;" % ", ".join("A%d" % r for r in range(4)))
-    for j in range(SB_D):
-        L.append("T%d: .branchtargets %s;" % (j, ", ".join("R%d_%d" % (j, v) for v in range(NO))))
-    L.append("brx.idx.uni %s, TA;" % AR)
-    for r in range(4):
-        L.append("A%d:" % r)
-        for m in range(NCHUNK):
-            off = 16 * (m + ((r + m) >> 2))   # padded layout: one pad chunk after every 4 (subband.cu sb_phys)
-            L.append("ld.shared.v2.b64 {w%d, w%d}, [%s+%d];" % (2 * m, 2 * m + 1, SA, off))
+    def tree(j, lo, hi, bit):
+        # binary decision tree over leaves [lo, hi) on bits bit..0 of o_j; the low half falls through
+        if hi - lo == 1:
+            return body(j, lo)
+        mid = lo + (1 << bit)
+        if mid >= hi:
+            return tree(j, lo, hi, bit - 1)
+        lab = "U%d_%d_%d" % (j, mid, bit)
+        return (["@q%d bra.uni %s;" % (bit, lab)] + tree(j, lo, mid, bit - 1) + ["%s:" % lab] + tree(j, mid, hi, bit - 1))
+
+    def after_loads():
+        out = []
+        if dispatch == "brx":
+            for j in range(D):
+                out.append("bfe.u32 t%d, %s, %d, 4;" % (j, OB, 4 * j))
+        else:
+            out += preds(0)
         for i in range(NW):
-            L.append("mov.b64 {l%d, h%d}, w%d;" % (i, i, i))
+            out.append("mov.b64 {l%d, h%d}, w%d;" % (i, i, i))
         for i in range(NV):
-            L.append("or.b32 x%d, h%d, %s;" % (i, i, ZERO))
-            L.append("or.b32 y%d, l%d, %s;" % (i, i + 1, ZERO))
-            L.append("mov.b64 v%d, {x%d, y%d};" % (i, i, i))
-        L += dispatch(0)
-    for j in range(SB_D):
-        for o in range(NO):
-            L.append("R%d_%d:" % (j, o))
-            for k in range(K2):
-                src = ("v%d" if o & 1 else "w%d") % ((o >> 1) + k)
-                L.append("add.rn.f32x2 %s, %s, %s;" % (acc(j, k), acc(j, k), src))
-            L += dispatch(j + 1) if j + 1 < SB_D else ["bra.uni DONE;"]
+            if shifted_copy:
+                out.append("or.b32 x%d, h%d, %s;" % (i, i, ZERO))
+                out.append("or.b32 y%d, l%d, %s;" % (i, i + 1, ZERO))
+                out.append("mov.b64 v%d, {x%d, y%d};" % (i, i, i))
+            else:
+                out.append("mov.b64 v%d, {h%d, l%d};" % (i, i, i + 1))
+        return out + goto_row(0)
+
+    if head == "brx":
+        # one jump on the pad phase ar into P copies of the loads with immediate offsets
+        L.append("brx.idx.uni %s, TA;" % AR)
+        for r in range(P):
+            L.append("LA%d:" % r)
+            for m in range(NCHUNK):
+                off = 16 * (m + (r + m) // P)       # padded layout (subband.cu sb_phys)
+                L.append("ld.shared.v2.b64 {w%d, w%d}, [%s+%d];" % (2 * m, 2 * m + 1, SA, off))
+            L += after_loads()
+    else:
+        # branch-free: chunk m sits at sa + 16*(m + m/P) + 16*[ar >= P - m%P]  (one pad chunk per P)
+        L.append(".reg .pred pa; .reg .b32 sx, b<%d>;" % P)
+        L.append("mov.b32 b0, %s;" % SA)
+        for rho in range(1, min(P, NCHUNK)):
+            L += ["setp.ge.u32 pa, %s, %d;" % (AR, P - rho), "selp.b32 sx, 16, 0, pa;", "add.u32 b%d, %s, sx;" % (rho, SA)]
+        for m in range(NCHUNK):
+            L.append("ld.shared.v2.b64 {w%d, w%d}, [b%d+%d];" % (2 * m, 2 * m + 1, m % P, 16 * (m + m // P)))
+        L += after_loads()
+    for j in range(D):
+        if dispatch == "brx":
+            for o in range(NO):
+                L += body(j, o)
+        else:
+            L.append("TREE%d:" % j)
+            L += tree(j, 0, NO, 3)
     L += ["DONE:", "}"]
     text = "\n".join('    "%s\\n"' % s for s in L)
-    outs = ", ".join('"+l"(acc[%d][%d])' % (j, k) for j in range(SB_D) for k in range(K2))
+    outs = ", ".join('"+l"(acc[%d][%d])' % (j, k) for j in range(D) for k in range(K2))
     ins = '"r"(sa), "r"(ar), "r"(obits), "r"(zero)'
-    head = ("// GENERATED by gen_subband_rows.py (SB_D=%d SB_K=%d SB_OMAX=%d) - do not edit.\n"
-            "// One channel of the SUBBAND kernel: window load (4 pad phases), shifted copy, 8 threaded row dispatches.\n"
-            % (SB_D, SB_K, SB_OMAX))
-    return head + "asm volatile(\n%s\n    : %s\n    : %s\n    : \"memory\");\n" % (text, outs, ins)
+    head = ("// GENERATED by gen_subband_rows.py %d %d %d %d - do not edit.\n"
+            "// One channel of the SUBBAND kernel: window load (%d pad phases), shifted pairs, %d threaded row dispatches.\n"
+            % (D, K, OMAX, shifted_copy, P, D))
+    params = ("#ifdef SB_ROWS_PARAMS\n"
+              "static_assert(SB_D == %d && SB_K == %d && SB_OMAX == %d, \"regenerate subband_rows.inc (gen_subband_rows.py)\");\n"
+              "#else\n" % (D, K, OMAX))
+    return head + params + "asm volatile(\n%s\n    : %s\n    : %s\n    : \"memory\");\n#endif\n" % (text, outs, ins)
 
 
 if __name__ == "__main__":
+    a = [int(x) for x in sys.argv[1:]]
+    D, K, OMAX = a[:3] if len(a) >= 3 else (4, 32, 12)
+    sc = a[3] if len(a) > 3 else 1
+    disp = "brx" if len(a) > 4 and a[4] == 1 else "tree"
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:
-        f.write(generate())
-    print(path)
+        f.write(generate(D, K, OMAX, sc, disp))
+    print(path, D, K, OMAX, sc)

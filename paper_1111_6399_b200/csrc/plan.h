@@ -19,16 +19,22 @@ struct TiledGeom {
 // SUBBAND kernel (subband.cu): exact sub-band re-skewed multi-pass with register-window reuse.
 // Thread tile = SB_D DM rows x SB_K consecutive samples; warp = one DM group (SB_D rows) x 32 lanes;
 // CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
-constexpr int SB_D = 8;
-constexpr int SB_K = 16;
+#ifndef SB_D_CFG
+#define SB_D_CFG 4
+#define SB_K_CFG 32
+#define SB_OMAX_CFG 12
+#endif
+constexpr int SB_D = SB_D_CFG;
+constexpr int SB_K = SB_K_CFG;
 constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
 constexpr int SB_WARPS = 8;           // DM groups per CTA
 constexpr int SB_ROWS = SB_D * SB_WARPS;
-constexpr int SB_OMAX = 12;           // largest in-window offset a row may have (switch cases 0..SB_OMAX)
-constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel (7)
+constexpr int SB_OMAX = SB_OMAX_CFG;  // largest in-window offset a row may have (bodies 0..SB_OMAX)
+constexpr int SB_P = SB_K / 4;        // 16-byte chunks per lane = pad period of the staged layout
+constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel
 constexpr int SB_CB = 8;              // channels per pipeline stage
 constexpr int SB_STAGES = 3;
-constexpr int SB_NCH_MAX = 224;       // staged chunks per channel the slot can hold (logical)
+constexpr int SB_NCH_MAX = SB_P * 32 + 96;  // staged chunks per channel the slot can hold (logical)
 
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;

@@ -72,7 +72,7 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
                     p->sb.records[(size_t)c * gslots + q] = rec;
                 }
             }
-            const int nch = amax + 4 * 31 + SB_WCHUNKS;
+            const int nch = amax + SB_P * 31 + SB_WCHUNKS;
             if (nch > SB_NCH_MAX || amax > 0xffff) return false;
             if (emit) {
                 p->sb.meta[((size_t)c * nblk + b) * 2 + 0] = rbase;
@@ -176,7 +176,7 @@ long long subband_verify_records(const dedisp_plan *p) {
                 const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
                 const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
                 const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 4 * a + o;
-                if (s != p->shifts[(size_t)c * ndm + d] || a + 4 * 31 + SB_WCHUNKS > nch || (rbase & 3)) ++bad;
+                if (s != p->shifts[(size_t)c * ndm + d] || a + SB_P * 31 + SB_WCHUNKS > nch || (rbase & 3) || o > SB_OMAX) ++bad;
             }
         }
     }
@@ -195,7 +195,11 @@ constexpr int SB_THREADS = SB_WARPS * 32;
 static_assert(SB_CB == SB_WARPS, "staging maps one warp to one channel of a stage");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
-__host__ __device__ constexpr int sb_phys(int chunk) { return chunk + (chunk >> 2); }  // 1 pad chunk per 4
+__host__ __device__ constexpr int sb_phys(int chunk) { return chunk + chunk / SB_P; }  // 1 pad chunk per SB_P
+static_assert((SB_P & (SB_P - 1)) == 0 && SB_P >= 2 && SB_D * 4 <= 32, "tile constants");
+#define SB_ROWS_PARAMS
+#include "subband_rows.inc"
+#undef SB_ROWS_PARAMS
 constexpr int SB_SLOT_CHUNKS_MAX = sb_phys(SB_NCH_MAX) + 1;
 
 __device__ __forceinline__ void sb_cp_async16_s(unsigned sa, const void *gmem) {
@@ -243,7 +247,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned stage_bytes = SB_CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
     uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
-    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 80u * lane;  // 5 chunks per lane (sb_phys)
+    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 16u * (SB_P + 1) * lane;  // sb_phys(SB_P * lane)
     const unsigned zero = A.zero;
 
     sb_u64 acc[SB_D][SB_K / 2];
@@ -256,7 +260,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const int nstages = (nchan + SB_CB - 1) / SB_CB;
 
     // Staging: warp w copies channel w of the stage (SB_CB == SB_WARPS); lane l copies logical chunks
-    // l, l+32, ... into the padded layout (sb_phys(l + 32 it) = sb_phys(l) + 40 it). All of a warp's
+    // l, l+32, ... into the padded layout (sb_phys(l + 32 it) = sb_phys(l) + sb_phys(32) it). All of a warp's
     // quantities but the lane term are warp-uniform; only windows that cross either end of the input
     // allocation take the bounds-checked zero-filling path.
     const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sdata);
@@ -267,19 +271,19 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const int buf = stage % SB_STAGES;
             const int2 mt = __ldg(meta2 + (size_t)c * A.nblk + blk);
             const long long e0 = (long long)c * A.in_stride + U0 + mt.x;
-            const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * (lane + (lane >> 2));
+            const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * sb_phys(lane);
             const float *src = in + e0 + 4 * lane;
             if (e0 >= 0 && e0 + 4ll * mt.y <= A.in_total) {
 #pragma unroll
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it)
-                    if (lane + 32 * it < mt.y) sb_cp_async16_s(dst + 640u * it, src + 128 * it);
+                    if (lane + 32 * it < mt.y) sb_cp_async16_s(dst + 16u * sb_phys(32) * it, src + 128 * it);
             } else {
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it) {
                     if (lane + 32 * it >= mt.y) break;
                     const long long e = e0 + 4 * lane + 128ll * it;
                     long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
                     valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
-                    sb_cp_async16_zs(dst + 640u * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
+                    sb_cp_async16_zs(dst + 16u * sb_phys(32) * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
                 }
             }
             if (lane < 4)   // the 8 warps' records of this channel: 64 contiguous bytes
@@ -299,12 +303,14 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         const int nch = min(SB_CB, nchan - stage * SB_CB);
         const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
         unsigned slot_u32 = sdata_u32 + buf * stage_bytes;
+        uint2 rec_next = *recp;                            // record of channel ch+1 is fetched one channel ahead
 #pragma unroll 1
-        for (int ch = 0; ch < nch; ++ch, recp += SB_WARPS, slot_u32 += slot_bytes) {
-            const uint2 rec = *recp;                       // warp-uniform: x = eight 4-bit o_j, y = chunk base a
+        for (int ch = 0; ch < nch; ++ch, slot_u32 += slot_bytes) {
+            const uint2 rec = rec_next;                    // warp-uniform: x = SB_D 4-bit o_j, y = chunk base a
+            rec_next = recp[min(ch + 1, SB_CB - 1) * SB_WARPS];
             const unsigned obits = rec.x;
-            const unsigned ar = rec.y & 3u;
-            const unsigned sa = slot_u32 + ((rec.y + (rec.y >> 2)) << 4);
+            const unsigned ar = rec.y & (unsigned)(SB_P - 1);
+            const unsigned sa = slot_u32 + ((rec.y + rec.y / SB_P) << 4);
 #include "subband_rows.inc"
         }
         __syncthreads();
