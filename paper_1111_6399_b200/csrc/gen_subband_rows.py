@@ -138,8 +138,8 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
 
 if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
-    D, K, OMAX = a[:3] if len(a) >= 3 else (4, 32, 12)
-    sc = a[3] if len(a) > 3 else 1
+    D, K, OMAX = a[:3] if len(a) >= 3 else (3, 32, 12)
+    sc = a[3] if len(a) > 3 else 0
     disp = "brx" if len(a) > 4 and a[4] == 1 else "tree"
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:

@@ -20,14 +20,17 @@ struct TiledGeom {
 // Thread tile = SB_D DM rows x SB_K consecutive samples; warp = one DM group (SB_D rows) x 32 lanes;
 // CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
 #ifndef SB_D_CFG
-#define SB_D_CFG 4
+#define SB_D_CFG 3
 #define SB_K_CFG 32
 #define SB_OMAX_CFG 12
+#endif
+#ifndef SB_WARPS_CFG
+#define SB_WARPS_CFG 12
 #endif
 constexpr int SB_D = SB_D_CFG;
 constexpr int SB_K = SB_K_CFG;
 constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
-constexpr int SB_WARPS = 8;           // DM groups per CTA
+constexpr int SB_WARPS = SB_WARPS_CFG; // DM groups per CTA (one warp each)
 constexpr int SB_ROWS = SB_D * SB_WARPS;
 constexpr int SB_OMAX = SB_OMAX_CFG;  // largest in-window offset a row may have (bodies 0..SB_OMAX)
 constexpr int SB_P = SB_K / 4;        // 16-byte chunks per lane = pad period of the staged layout

@@ -192,11 +192,11 @@ long long subband_verify_records(const dedisp_plan *p) {
 namespace {
 
 constexpr int SB_THREADS = SB_WARPS * 32;
-static_assert(SB_CB == SB_WARPS, "staging maps one warp to one channel of a stage");
+static_assert(SB_CB <= SB_WARPS, "staging maps one warp to one channel of a stage");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
 __host__ __device__ constexpr int sb_phys(int chunk) { return chunk + chunk / SB_P; }  // 1 pad chunk per SB_P
-static_assert((SB_P & (SB_P - 1)) == 0 && SB_P >= 2 && SB_D * 4 <= 32, "tile constants");
+static_assert((SB_P & (SB_P - 1)) == 0 && SB_P >= 2 && SB_D * 4 <= 32 && SB_WARPS % 2 == 0, "tile constants");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
 #undef SB_ROWS_PARAMS
@@ -265,40 +265,51 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     // allocation take the bounds-checked zero-filling path.
     const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sdata);
     const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
+    // meta (window base, chunk count) of the channel this warp stages next: loaded one stage ahead so
+    // that its L2 latency never sits in front of the copies
+    auto load_meta = [&](int stage) -> int2 {
+        const int c = A.c_begin + stage * SB_CB + warp;
+        if (stage < nstages && warp < SB_CB && c < A.c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
+        return make_int2(0, 0);
+    };
+    int2 mt = load_meta(0);
     auto issue = [&](int stage) {
         const int c = A.c_begin + stage * SB_CB + warp;
-        if (stage < nstages && c < A.c_end) {
+        const int2 mt_cur = mt;
+        mt = load_meta(stage + 1);
+        if (stage < nstages && warp < SB_CB && c < A.c_end) {
             const int buf = stage % SB_STAGES;
-            const int2 mt = __ldg(meta2 + (size_t)c * A.nblk + blk);
-            const long long e0 = (long long)c * A.in_stride + U0 + mt.x;
+            const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
             const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * sb_phys(lane);
             const float *src = in + e0 + 4 * lane;
-            if (e0 >= 0 && e0 + 4ll * mt.y <= A.in_total) {
+            if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
 #pragma unroll
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it)
-                    if (lane + 32 * it < mt.y) sb_cp_async16_s(dst + 16u * sb_phys(32) * it, src + 128 * it);
+                    if (lane + 32 * it < mt_cur.y) sb_cp_async16_s(dst + 16u * sb_phys(32) * it, src + 128 * it);
             } else {
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it) {
-                    if (lane + 32 * it >= mt.y) break;
+                    if (lane + 32 * it >= mt_cur.y) break;
                     const long long e = e0 + 4 * lane + 128ll * it;
                     long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
                     valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
                     sb_cp_async16_zs(dst + 16u * sb_phys(32) * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
                 }
             }
-            if (lane < 4)   // the 8 warps' records of this channel: 64 contiguous bytes
+            if (lane < SB_WARPS / 2)   // the SB_WARPS records of this channel: contiguous, 16-byte aligned
                 sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * SB_CB + warp) * SB_WARPS) + 16u * lane,
                                 reinterpret_cast<const char *>(A.records + (size_t)c * A.gslots + blk * SB_WARPS) + 16 * lane);
         }
         sb_commit();
     };
 
+    // 3-stage ring, one barrier per stage: after the barrier every warp has finished stage-1, so its
+    // buffer can be refilled with stage+2 while stage is consumed.
     issue(0);
     issue(1);
     for (int stage = 0; stage < nstages; ++stage) {
-        issue(stage + 2);
-        sb_wait<2>();
+        sb_wait<1>();
         __syncthreads();
+        issue(stage + 2);
         const int buf = stage % SB_STAGES;
         const int nch = min(SB_CB, nchan - stage * SB_CB);
         const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
@@ -313,7 +324,6 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const unsigned sa = slot_u32 + ((rec.y + rec.y / SB_P) << 4);
 #include "subband_rows.inc"
         }
-        __syncthreads();
     }
 
     OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
