@@ -40,7 +40,7 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
         return "%%%d" % (j * K2 + k)
 
     SA, AR, OB, ZERO = ("%%%d" % (D * K2 + i) for i in range(4))
-    L = ["{", ".reg .b32 t<%d>, tt;" % D, ".reg .pred q<4>;", ".reg .b64 w<%d>, v<%d>;" % (NW, NV),
+    L = ["{", ".reg .f32 al, ah, lf<%d>, hf<%d>;" % (NW, NW), ".reg .b32 t<%d>, tt;" % D, ".reg .pred q<4>;", ".reg .b64 w<%d>, v<%d>;" % (NW, NV),
          ".reg .b32 l<%d>, h<%d>, x<%d>, y<%d>;" % (NW, NW, NV, NV)]
     if head == "brx":
         L.append("TA: .branchtargets %s;" % ", ".join("LA%d" % r for r in range(P)))
@@ -66,8 +66,15 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
         if dispatch == "tree" and j + 1 < D:
             out += preds(j + 1)
         for k in range(K2):
-            src = ("v%d" if o & 1 else "w%d") % ((o >> 1) + k)
-            out.append("add.rn.f32x2 %s, %s, %s;" % (acc(j, k), acc(j, k), src))
+            if (o & 1) and shifted_copy == 2:
+                # odd offset, no shifted copy: two scalar FADDs on the halves of the accumulator pair
+                # (same fp32-pipe time as one FADD2, one more issue slot, no moves, no extra registers)
+                i = (o >> 1) + k
+                out += ["mov.b64 {al, ah}, %s;" % acc(j, k), "add.rn.f32 al, al, hf%d;" % i,
+                        "add.rn.f32 ah, ah, lf%d;" % (i + 1), "mov.b64 %s, {al, ah};" % acc(j, k)]
+            else:
+                src = ("v%d" if o & 1 else "w%d") % ((o >> 1) + k)
+                out.append("add.rn.f32x2 %s, %s, %s;" % (acc(j, k), acc(j, k), src))
         return out + goto_row(j + 1)
 
     def tree(j, lo, hi, bit):
@@ -89,6 +96,10 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
             out += preds(0)
         for i in range(NW):
             out.append("mov.b64 {l%d, h%d}, w%d;" % (i, i, i))
+        if shifted_copy == 2:
+            for i in range(NW):
+                out.append("mov.b64 {lf%d, hf%d}, w%d;" % (i, i, i))
+            return out + goto_row(0)
         for i in range(NV):
             if shifted_copy:
                 out.append("or.b32 x%d, h%d, %s;" % (i, i, ZERO))
@@ -139,7 +150,7 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
 if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
     D, K, OMAX = a[:3] if len(a) >= 3 else (3, 32, 12)
-    sc = a[3] if len(a) > 3 else 0
+    sc = a[3] if len(a) > 3 else 2
     disp = "brx" if len(a) > 4 and a[4] == 1 else "tree"
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:
