@@ -36,7 +36,10 @@ constexpr int SB_OMAX = SB_OMAX_CFG;  // largest in-window offset a row may have
 constexpr int SB_P = SB_K / 4;        // 16-byte chunks per lane = pad period of the staged layout
 constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel
 constexpr int SB_CB = 8;              // channels per pipeline stage
-constexpr int SB_STAGES = 3;
+#ifndef SB_STAGES_CFG
+#define SB_STAGES_CFG 4
+#endif
+constexpr int SB_STAGES = SB_STAGES_CFG;
 constexpr int SB_NCH_MAX = SB_P * 32 + 96;  // staged chunks per channel the slot can hold (logical)
 
 struct SubbandPass {

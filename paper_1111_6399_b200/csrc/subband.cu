@@ -302,14 +302,14 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         sb_commit();
     };
 
-    // 3-stage ring, one barrier per stage: after the barrier every warp has finished stage-1, so its
-    // buffer can be refilled with stage+2 while stage is consumed.
-    issue(0);
-    issue(1);
+    // SB_STAGES-deep ring, one barrier per stage: after the barrier every warp has finished stage-1, so
+    // its buffer can be refilled with stage+SB_STAGES-1 while stage is consumed.
+#pragma unroll
+    for (int st = 0; st < SB_STAGES - 1; ++st) issue(st);
     for (int stage = 0; stage < nstages; ++stage) {
-        sb_wait<1>();
+        sb_wait<SB_STAGES - 2>();
         __syncthreads();
-        issue(stage + 2);
+        issue(stage + SB_STAGES - 1);
         const int buf = stage % SB_STAGES;
         const int nch = min(SB_CB, nchan - stage * SB_CB);
         const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
