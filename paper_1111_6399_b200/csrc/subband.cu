@@ -326,18 +326,35 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         }
     }
 
-    OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
+    // Epilogue: a lane holds SB_K consecutive samples of each row, so direct stores would touch 32
+    // sectors per instruction. Transpose through the (now idle) ring: each warp parks its tile in its
+    // own padded region and writes / read-modify-writes out[d][t] with lanes on consecutive samples.
+    sb_wait<0>();
+    __syncthreads();
+    constexpr int EP_PITCH = SB_K + 4;                       // words per lane: 16-byte aligned, odd number of chunks
+    float *ep = reinterpret_cast<float *>(sb_smem) + (size_t)warp * (SB_D * 32 * EP_PITCH);
 #pragma unroll
+    for (int j = 0; j < SB_D; ++j)
+#pragma unroll
+        for (int k4 = 0; k4 < SB_K / 4; ++k4) {
+            const sb_u64 p0 = acc[j][2 * k4], p1 = acc[j][2 * k4 + 1];
+            *reinterpret_cast<uint4 *>(ep + (j * 32 + lane) * EP_PITCH + 4 * k4) =
+                make_uint4((unsigned)p0, (unsigned)(p0 >> 32), (unsigned)p1, (unsigned)(p1 >> 32));
+        }
+    __syncwarp();
+    OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
+#pragma unroll 1
     for (int j = 0; j < SB_D; ++j) {
         const int d = d_first + warp * SB_D + j;
-        if (d >= A.ndm) continue;
-        const long long t0 = U0 + SB_K * lane - (long long)__ldg(A.skew + d);
+        if (d >= A.ndm) break;
+        const long long t0 = U0 - (long long)__ldg(A.skew + d);
         OutT *orow = out + (size_t)d * A.out_stride;
-#pragma unroll
-        for (int k = 0; k < SB_K; ++k) {
-            const long long t = t0 + k;
-            const unsigned bits = (k & 1) ? (unsigned)(acc[j][k >> 1] >> 32) : (unsigned)acc[j][k >> 1];
-            const float v = __uint_as_float(bits);
+        const float *erow = ep + j * 32 * EP_PITCH;
+#pragma unroll 8
+        for (int i = 0; i < SB_K; ++i) {
+            const int sidx = i * 32 + lane;                  // sample within the tile, lanes consecutive
+            const float v = erow[(sidx / SB_K) * EP_PITCH + (sidx % SB_K)];
+            const long long t = t0 + sidx;
             if (t >= 0 && t < A.nsamp_out) {
                 if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
                     const int vi = __float2int_rn(v);
@@ -459,7 +476,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.gslots = sb.nblk * SB_WARPS;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
-    const size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8;
+    size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8;
+    smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * (SB_K + 4) * sizeof(float));  // epilogue transpose region
     auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
