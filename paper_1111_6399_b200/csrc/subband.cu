@@ -152,6 +152,8 @@ void subband_build(dedisp_plan *p) {
         std::memcpy(sb.skew.data() + g * (size_t)ndm, sref, (size_t)ndm * sizeof(int32_t));
         ps.max_skew = sref[ndm - 1];
     }
+    // the kernel's dynamic shared memory (ring + records) must fit the 227 KB a CTA may opt into
+    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + sb.max_nch / SB_P + 1) * 16 + SB_WARPS * 8) > 227u * 1024u) { sb = SubbandGeom(); return; }
     sb.ok = true;
 }
 
