@@ -59,11 +59,28 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
     def goto_row(j):
         if j >= D:
             return ["bra.uni DONE;"]
-        return ["brx.idx.uni t%d, T%d;" % (j, j)] if dispatch == "brx" else ["bra.uni TREE%d;" % j]
+        if dispatch == "brx":
+            return ["brx.idx.uni t%d, T%d;" % (j, j)]
+        if dispatch == "ttree":
+            uid[0] += 1
+            return jump_tree(j, 0, NO, 3, "c%d" % uid[0])   # private copy of row j's decision tree: no merge point
+        return ["bra.uni TREE%d;" % j]
+
+    uid = [0]
+
+    def jump_tree(j, lo, hi, bit, tag):
+        # decision tree whose leaves are jumps to the shared bodies R<j>_<o>
+        if hi - lo == 1:
+            return ["bra.uni R%d_%d;" % (j, lo)]
+        mid = lo + (1 << bit)
+        if mid >= hi:
+            return jump_tree(j, lo, hi, bit - 1, tag)
+        lab = "V%s_%d_%d_%d" % (tag, j, mid, bit)
+        return (["@q%d bra.uni %s;" % (bit, lab)] + jump_tree(j, lo, mid, bit - 1, tag) + ["%s:" % lab] + jump_tree(j, mid, hi, bit - 1, tag))
 
     def body(j, o):
         out = ["R%d_%d:" % (j, o)]
-        if dispatch == "tree" and j + 1 < D:
+        if dispatch in ("tree", "ttree") and j + 1 < D:
             out += preds(j + 1)
         for k in range(K2):
             if (o & 1) and shifted_copy == 2:
@@ -128,7 +145,7 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
             L.append("ld.shared.v2.b64 {w%d, w%d}, [b%d+%d];" % (2 * m, 2 * m + 1, m % P, 16 * (m + m // P)))
         L += after_loads()
     for j in range(D):
-        if dispatch == "brx":
+        if dispatch in ("brx", "ttree"):
             for o in range(NO):
                 L += body(j, o)
         else:
@@ -151,7 +168,7 @@ if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
     D, K, OMAX = a[:3] if len(a) >= 3 else (3, 32, 12)
     sc = a[3] if len(a) > 3 else 2
-    disp = "brx" if len(a) > 4 and a[4] == 1 else "tree"
+    disp = {0: "tree", 1: "brx", 2: "ttree"}[a[4] if len(a) > 4 else 0]
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:
         f.write(generate(D, K, OMAX, sc, disp))

@@ -36,11 +36,11 @@ constexpr int SB_OMAX = SB_OMAX_CFG;  // largest in-window offset a row may have
 constexpr int SB_P = SB_K / 4;        // 16-byte chunks per lane = pad period of the staged layout
 constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel
 #ifndef SB_CB_CFG
-#define SB_CB_CFG 12
+#define SB_CB_CFG 8
 #endif
 constexpr int SB_CB = SB_CB_CFG;      // channels per pipeline stage (one staging warp each)
 #ifndef SB_STAGES_CFG
-#define SB_STAGES_CFG 3
+#define SB_STAGES_CFG 4
 #endif
 constexpr int SB_STAGES = SB_STAGES_CFG;
 constexpr int SB_NCH_MAX = SB_P * 32 + 96;  // staged chunks per channel the slot can hold (logical)

@@ -153,7 +153,7 @@ void subband_build(dedisp_plan *p) {
         ps.max_skew = sref[ndm - 1];
     }
     // the kernel's dynamic shared memory (ring + records) must fit the 227 KB a CTA may opt into
-    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + sb.max_nch / SB_P + 1) * 16 + SB_WARPS * 8) > 227u * 1024u) { sb = SubbandGeom(); return; }
+    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + sb.max_nch / SB_P + 1) * 16 + SB_WARPS * 8 + 16) > 227u * 1024u) { sb = SubbandGeom(); return; }
     sb.ok = true;
 }
 
@@ -209,6 +209,19 @@ __device__ __forceinline__ void sb_cp_async16_s(unsigned sa, const void *gmem) {
 }
 __device__ __forceinline__ void sb_cp_async16_zs(unsigned sa, const void *gmem, int src_bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void sb_mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void sb_mbar_arrive(unsigned bar) {
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (pending count unchanged)
+__device__ __forceinline__ void sb_mbar_arrive_cp_async(unsigned bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void sb_mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n@p bra.uni DONE_%=;\nbra.uni WAIT_%=;\nDONE_%=:\n}\n" ::"r"(bar), "r"(parity) : "memory");
 }
 __device__ __forceinline__ void sb_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void sb_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
@@ -301,17 +314,33 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                 sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * SB_CB + warp) * SB_WARPS) + 16u * lane,
                                 reinterpret_cast<const char *>(A.records + (size_t)c * A.gslots + blk * SB_WARPS) + 16 * lane);
         }
-        sb_commit();
     };
 
-    // SB_STAGES-deep ring, one barrier per stage: after the barrier every warp has finished stage-1, so
-    // its buffer can be refilled with stage+SB_STAGES-1 while stage is consumed.
+    // SB_STAGES-deep ring without CTA-wide barriers: full[b] completes when every thread's copies of
+    // the stage in buffer b have landed, empty[b] when every warp has finished reading it. A stage is
+    // refilled SB_DIST = SB_STAGES - 2 stages ahead, i.e. into the buffer read two stages ago, so a
+    // fast warp can run one whole stage ahead of the slowest before it has to wait.
+    constexpr int SB_DIST = SB_STAGES - 2;
+    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + SB_STAGES * SB_CB * SB_WARPS);
+    const unsigned bar_empty = bar_full + 8u * SB_STAGES;
+    if (tid == 0) {
 #pragma unroll
-    for (int st = 0; st < SB_STAGES - 1; ++st) issue(st);
+        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, SB_THREADS); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int st = 0; st < SB_DIST; ++st) { issue(st); sb_mbar_arrive_cp_async(bar_full + 8u * (st % SB_STAGES)); }
     for (int stage = 0; stage < nstages; ++stage) {
-        sb_wait<SB_STAGES - 2>();
-        __syncthreads();
-        issue(stage + SB_STAGES - 1);
+        const int pst = stage + SB_DIST;
+        if (pst < nstages) {
+            const int pb = pst % SB_STAGES;
+            if (pst >= SB_STAGES) sb_mbar_wait(bar_empty + 8u * pb, (unsigned)((pst / SB_STAGES - 1) & 1));
+            issue(pst);
+            sb_mbar_arrive_cp_async(bar_full + 8u * pb);
+        } else {
+            mt = make_int2(0, 0);
+        }
+        sb_mbar_wait(bar_full + 8u * (stage % SB_STAGES), (unsigned)((stage / SB_STAGES) & 1));
         const int buf = stage % SB_STAGES;
         const int nch = min(SB_CB, nchan - stage * SB_CB);
         const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
@@ -326,12 +355,13 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const unsigned sa = slot_u32 + ((rec.y + rec.y / SB_P) << 4);
 #include "subband_rows.inc"
         }
+        __syncwarp();
+        if (lane == 0) sb_mbar_arrive(bar_empty + 8u * (stage % SB_STAGES));
     }
 
     // Epilogue: a lane holds SB_K consecutive samples of each row, so direct stores would touch 32
     // sectors per instruction. Transpose through the (now idle) ring: each warp parks its tile in its
     // own padded region and writes / read-modify-writes out[d][t] with lanes on consecutive samples.
-    sb_wait<0>();
     __syncthreads();
     constexpr int EP_PITCH = SB_K + 4;                       // words per lane: 16-byte aligned, odd number of chunks
     float *ep = reinterpret_cast<float *>(sb_smem) + (size_t)warp * (SB_D * 32 * EP_PITCH);
@@ -478,7 +508,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.gslots = sb.nblk * SB_WARPS;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
-    size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8;
+    size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8 + 16 * SB_STAGES;
     smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * (SB_K + 4) * sizeof(float));  // epilogue transpose region
     auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
