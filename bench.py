@@ -36,6 +36,27 @@ def _peaks():
     return 6650.0, 1965.0, "fallback"
 
 
+def beam_seed(cfg_seed: int, rank: int) -> int:
+    """Each rank de-disperses its own synthetic beam (independent problems: DESIGN.md section 9)."""
+    return cfg_seed + 7919 * rank
+
+
+def max_over_ranks(x: float, world: int, device="cuda") -> float:
+    """Slowest rank's time: the whole-job time of a sharded run (contract: max over ranks)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(adds_per_rank: int, steps: int, world: int, slowest_seconds: float) -> float:
+    """Whole-job Gadds/s: every rank did adds_per_rank*steps adds in the slowest rank's time."""
+    return world * adds_per_rank * steps / slowest_seconds / 1e9
+
+
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -156,12 +177,8 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    def max_over(x: float) -> float:
+        return max_over_ranks(x, world)
 
     hbm_gbs, sm_max_mhz, peak_src = _peaks()
     plan = P.Plan.from_config(cfg)                      # table build + upload: once per plan, not per step
@@ -169,7 +186,7 @@ def run_ours(args, cfg):
         plan.set_kernel({"naive": 1, "tiled": 2, "subband": 3}[args.kernel])
     nsamp_in = cfg.nsamp_out + plan.max_shift
     # each rank de-disperses its own beam (independent problems, no data-path collective): weak scaling
-    x, _ = synth.make_input(cfg, plan.shifts(), nsamp_in, device="cuda", seed=cfg.seed + 7919 * rank)
+    x, _ = synth.make_input(cfg, plan.shifts(), nsamp_in, device="cuda", seed=beam_seed(cfg.seed, rank))
     out = plan.alloc_out(cfg.nsamp_out)
     adds = cfg.ndm * cfg.nchans * cfg.nsamp_out
     launches = plan.launches_per_execute
@@ -188,9 +205,9 @@ def run_ours(args, cfg):
         b.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = max_over_ranks(evs[0][0].elapsed_time(evs[-1][1]))
+    total_ms = max_over(evs[0][0].elapsed_time(evs[-1][1]))
     step_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps       # device time of one execute
-    value = world * adds * args.steps / (total_ms * 1e-3) / 1e9
+    value = job_value(adds, args.steps, world, total_ms * 1e-3)
 
     # ---- e2e: the host-buffer C-ABI call; H2D + kernels + D2H inside the timed region
     e2e = None
@@ -205,8 +222,8 @@ def run_ours(args, cfg):
         for _ in range(esteps):
             plan.execute_host(h_in, cfg.nsamp_out, h_out)
         barrier()
-        et = max_over_ranks(time.perf_counter() - t0)
-        e2e = {"value": world * adds * esteps / et / 1e9, "unit": UNIT,
+        et = max_over(time.perf_counter() - t0)
+        e2e = {"value": job_value(adds, esteps, world, et), "unit": UNIT,
                "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
                "d2h_bytes_per_step": h_out.numel() * h_out.element_size(), "steps": esteps,
                "ms_per_step": 1e3 * et / esteps, "api": "dedisp_execute_host (pinned host buffers)"}
