@@ -271,13 +271,100 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+def run_c5_stream(args, cfg):
+    """c5 (configs[4]): 32 beams x 1024 ch u8, consecutive 32768-sample chunks through the streaming
+    driver. value = one chunk of all beams, inputs resident (dedisp_execute_batched); e2e = chunks
+    pushed from pinned host memory through dedisp_stream_push (H2D overlapped with compute, maxshift
+    carry on the device), reading back the per-(beam, DM) maximum of every block. 1 GPU only."""
+    import torch
+
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import synth
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product has no CPU path"
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    hbm_gbs, sm_max_mhz, peak_src = _peaks()
+    plan = P.Plan.from_config(cfg)
+    nb, chunk = cfg.nbeams, cfg.nsamp_out
+    nsamp_in = chunk + plan.max_shift
+    tab = plan.shifts()
+    xs = torch.empty((nb, cfg.nchans, nsamp_in), dtype=torch.uint8, device="cuda")
+    for b in range(nb):
+        xs[b], _ = synth.make_input(cfg, tab, nsamp_in, device="cuda", seed=cfg.seed * 1000003 + b * 101)
+    out = plan.alloc_out(chunk, nb)
+    adds = nb * cfg.ndm * cfg.nchans * chunk
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        plan.execute(xs, chunk, out)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    torch.cuda.synchronize()
+    sampler.start()
+    for a, b in evs:
+        a.record(stream)
+        plan.execute(xs, chunk, out)
+        b.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    total_ms = evs[0][0].elapsed_time(evs[-1][1])
+    step_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
+    value = adds * args.steps / (total_ms * 1e-3) / 1e9
+    del out
+    # ---- e2e: the streaming driver, a pool of 3 distinct pinned chunks cycled (generation is outside the timed region)
+    pool = [xs[:, :, plan.max_shift - k * 4096: plan.max_shift - k * 4096 + chunk].contiguous().cpu().pin_memory() for k in range(3)]
+    del xs
+    torch.cuda.empty_cache()
+    st = P.Stream(plan, nb, chunk, 3)                     # 3 buffers: block k-1 is still being read while k+1 is enqueued
+    esteps = max(args.steps, 6)
+    h_max = torch.empty((esteps, nb, cfg.ndm), dtype=torch.int32, pin_memory=True)
+    for k in range(2):                                   # warm-up pushes (fills the history)
+        st.push(pool[k % 3])
+    st.sync()
+    t0 = time.perf_counter()
+    prev = None
+    for k in range(esteps):
+        ptr, ev = st.push(pool[k % 3])
+        if prev is not None:                             # read block k-1's metric while block k computes
+            st.wait_event(prev[1])
+            h_max[k - 1].copy_(st.out_view(prev[0]).amax(dim=2), non_blocking=True)
+        prev = (ptr, ev)
+    st.wait_event(prev[1])
+    h_max[esteps - 1].copy_(st.out_view(prev[0]).amax(dim=2), non_blocking=True)
+    torch.cuda.synchronize()
+    et = time.perf_counter() - t0
+    st.close()
+    e2e = {"value": adds * esteps / et / 1e9, "unit": UNIT, "h2d_bytes_per_step": pool[0].numel(),
+           "d2h_bytes_per_step": nb * cfg.ndm * 4, "steps": esteps, "ms_per_step": 1e3 * et / esteps,
+           "real_time_factor": chunk * cfg.tsamp / (et / esteps),
+           "api": "dedisp_stream_push (pinned host chunks, 3 device buffers); D2H = per-(beam, DM) maxima of each block"}
+    peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6 / 1e9
+    achieved = adds / (step_ms * 1e-3) / 1e9
+    kname = {1: "naive", 2: "tiled", 3: "subband"}[plan.kernel]
+    bytes_once = nb * (cfg.nchans * nsamp_in + cfg.ndm * chunk * 4)
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kname)), "kernel": f"dedisp_{kname}_kernel",
+                "launches_per_step": plan.launches_per_execute,
+                "peak_source": f"148 SMs x 128 lanes x sm_max_mhz ({peak_src} MEASURED_PEAKS.json clock)",
+                "hbm_bytes_once": bytes_once, "hbm_time_ms_at_peak": bytes_once / (hbm_gbs * 1e9) * 1e3}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "i32", "data": "synthetic",
+            "config": {"workload": cfg.name, "nchans": cfg.nchans, "ndm": cfg.ndm, "nsamp_out": chunk, "nbeams": nb,
+                       "in_dtype": "u8", "l2": "input larger than L2, no flush", "kernel": kname,
+                       "note": "step = one 32768-sample chunk of all 32 beams"},
+            "real_time_factor": chunk * cfg.tsamp / (total_ms / args.steps * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_execute * args.steps,
+            "roofline": roofline, "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--kernel", default=None, choices=["naive", "tiled", "subband"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -289,6 +376,8 @@ def main():
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.config == "c5":
+        run_c5_stream(args, cfg)
     else:
         run_ours(args, cfg)
 

@@ -151,6 +151,10 @@ int dedisp_stream_create(dedisp_stream **s, dedisp_plan *plan, int nbeams, long 
  * [beam][ndm][chunk_nsamp], owned by the stream object, reused after nbuffers pushes) is valid
  * once *done_event (a cudaEvent_t as void*) has completed or after dedisp_stream_sync. */
 int dedisp_stream_push(dedisp_stream *s, const void *h_chunk, void **d_out, void **done_event);
+/* dedisp_stream_wait_event: make the caller's `stream` (cudaStream_t as void*) wait, on the device,
+ * for a done_event returned by dedisp_stream_push, so that work queued on it afterwards may read
+ * the block without a host synchronisation. EINVAL on a NULL event. */
+int dedisp_stream_wait_event(void *done_event, void *stream);
 int dedisp_stream_sync(dedisp_stream *s);
 int dedisp_stream_destroy(dedisp_stream *s);
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
     "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_error_string",
-    "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_sync",
+    "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
 
@@ -75,6 +75,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_last_cuda_error.restype = ctypes.c_char_p
         L.dedisp_stream_create.argtypes = [ctypes.POINTER(vp), vp, c_int, c_ll, c_int]
         L.dedisp_stream_push.argtypes = [vp, vp, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+        L.dedisp_stream_wait_event.argtypes = [vp, vp]
         L.dedisp_stream_sync.argtypes = [vp]
         L.dedisp_stream_destroy.argtypes = [vp]
         _lib = L
@@ -244,6 +245,10 @@ class Stream:
         """Zero-copy torch view ``[beam][ndm][chunk]`` of an output block owned by the stream object."""
         typestr = "<i4" if self.plan.dtype == U8 else "<f4"
         return torch.as_tensor(_DeviceBlob(out_ptr, (self.nbeams, self.plan.ndm, self.chunk), typestr), device="cuda")
+
+    def wait_event(self, event_ptr: int, stream=None) -> None:
+        """``dedisp_stream_wait_event``: ``stream`` (default: torch's current) waits for a block's done event."""
+        self.plan._check(lib().dedisp_stream_wait_event(event_ptr, _stream_ptr(stream)), "dedisp_stream_wait_event")
 
     def sync(self) -> None:
         self.plan._check(lib().dedisp_stream_sync(self._h), "dedisp_stream_sync")

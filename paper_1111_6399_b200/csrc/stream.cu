@@ -127,6 +127,11 @@ int dedisp_stream_push(dedisp_stream *s, const void *h_chunk, void **d_out, void
     return DEDISP_OK;
 }
 
+int dedisp_stream_wait_event(void *done_event, void *stream) {
+    if (!done_event) return DEDISP_EINVAL;
+    return cudaStreamWaitEvent((cudaStream_t)stream, (cudaEvent_t)done_event, 0) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+}
+
 int dedisp_stream_sync(dedisp_stream *s) {
     if (!s) return DEDISP_EINVAL;
     cudaError_t e = cudaStreamSynchronize(s->copy_st);
