@@ -1,29 +1,39 @@
 #!/usr/bin/env python
 """Generates ``subband_rows.inc`` — the per-channel body of the SUBBAND kernel (subband.cu) as one
-inline-PTX statement.  ``python gen_subband_rows.py [D K OMAX [shifted_copy]]`` after changing a
-tile constant; the generated file is committed so that the build needs nvcc only, and subband.cu
+inline-PTX statement.  ``python gen_subband_rows.py [D K OMAX [odd_mode [dispatch]]]`` after changing
+a tile constant; the generated file is committed so that the build needs nvcc only, and subband.cu
 static_asserts that its constants (plan.h) match the ones the file was generated for.
 
 Why PTX: a thread owns SB_D DM rows x SB_K consecutive samples and holds the union of its rows'
 input windows in registers; row j needs window words [o_j, o_j + SB_K) with o_j in 0..SB_OMAX known
-only at run time (warp-uniform).  Registers cannot be indexed dynamically, so each row jumps to one
-of SB_OMAX+1 bodies with static register operands.  Written as a C++ ``switch`` nvcc if-converts
-the bodies into select chains (13 predicated moves per add: measured 9.5 % of the add peak,
-profiles/r1_subband.md); written here as *threaded code* every body ends with the ``brx.idx`` of
-the NEXT row, which ptxas lowers to LDC (jump table) + BRX; the table indices of all rows are
-extracted when the channel starts so that the LDC can issue at the top of the previous body.
+only at run time (warp-uniform).  Registers cannot be indexed dynamically, so each row must reach one
+of SB_OMAX+1 bodies with static register operands.  Measured on c3 (profiles/r1_subband.md):
 
-Adds are ``add.rn.f32x2`` (SASS FADD2: two fp32 adds per lane per issue slot — the only way to
-leave issue slots for anything else at 128 lane-adds/clk/SM).  FADD2 needs its operands in aligned
-64-bit register pairs: even o_j use the window pairs as loaded (w), odd o_j use pairs shifted by
-one word (v).  With shifted_copy=1 the v pairs are built once per channel with ``or.b32 x, y, zero``
-(ALU pipe; ``zero`` is a run-time 0 so that ptxas cannot turn them into moves and sink them into
-every odd body); with shifted_copy=0 they are plain moves and ptxas sinks 2 moves per FADD2 into
-the odd bodies (fewer registers, more issue slots).
+  * a C++ ``switch`` is if-converted by nvcc into select chains (13 predicated moves per add): 9.5 %;
+  * dispatch 1, "brx": threaded code, every body ends with the ``brx.idx`` of the next row (LDC from
+    the jump table + BRX, ~88 cycles of warp latency per row): 15 %;
+  * dispatch 0, "tree" (committed): a binary tree of direct ``@q bra.uni`` on the four bits of o_j, the
+    predicates set one body ahead; a taken direct branch costs ~12 cycles;
+  * dispatch 2, "ttree": a private copy of the next row's tree in every body (no merge point, so no
+    BSSY/BSYNC per row) — larger code, measured 1 % slower.
 
-Operands of the statement:  %0.. acc[j][k2] (b64, "+l"), then sa (u32 shared address of the
-lane's first window chunk, already including the padded-layout term), ar (= a mod SB_K/4: which pad
-phase the window starts in), obits (SB_D 4-bit o_j), zero.
+Adds are ``add.rn.f32x2`` (SASS FADD2: two fp32 adds per lane per issue slot).  FADD2 needs aligned
+64-bit register pairs, which the window pairs as loaded provide for even o_j only.  Odd o_j:
+
+  * odd_mode 1: a copy shifted by one word, built once per channel with ``or.b32 x, y, zero`` (``zero``
+    is a run-time 0 so ptxas cannot turn the ORs into moves and sink them into every odd body);
+    costs 2*NCHUNK*2 registers and ALU-pipe time;
+  * odd_mode 0: plain moves; ptxas sinks 2 IMAD.MOV per FADD2 into the odd bodies — they run on the
+    fp32 pipe and steal its cycles;
+  * odd_mode 2 (committed): two scalar ``add.rn.f32`` on the halves of the accumulator pair — the same
+    fp32-pipe time as one FADD2, one more issue slot, no moves, no extra registers (this is what
+    lets 3 warps per scheduler fit: 168 registers).
+
+The window's pad phase (where in the padded shared-memory layout the lane's first chunk falls) is
+handled branch-free: chunk m sits at sa + 16*(m + m/P) + 16*[ar >= P - m%P].
+
+Operands of the statement:  %0.. acc[j][k2] (b64, "+l"), then sa (u32 shared address of the lane's
+first window chunk), ar (= a mod SB_K/4), obits (SB_D 4-bit o_j), zero.
 """
 import os
 import sys
