@@ -15,10 +15,12 @@
 // r(c,d) = s(c,d) - s(c_ref,d) varies by <= SB_OMAX-3 samples across a thread's SB_D rows.
 // One kernel launch per sub-band ("pass"); pass 0 stores, later passes add into out.
 //
-// Per channel a thread: 1 broadcast LDS of its record, SB_WCHUNKS LDS.128 of the window, then for
-// each of its SB_D rows a warp-uniform jump on the row's offset o_j into SB_K/2 FADD2 with static
-// register operands (registers cannot be indexed dynamically). That body is generated inline PTX:
-// see gen_subband_rows.py for why and subband_rows.inc for the text.
+// Per channel a thread: its record (prefetched one channel ahead), SB_WCHUNKS LDS.128 of the window,
+// then for each of its SB_D rows a warp-uniform tree of direct branches on the row's offset o_j into
+// a body with static register operands (registers cannot be indexed dynamically): SB_K/2 FADD2 for
+// even o_j, SB_K scalar FADD for odd o_j. That body is generated inline PTX: see gen_subband_rows.py
+// for why and subband_rows.inc for the text. Around it: an SB_STAGES-deep cp.async ring handed over
+// with mbarrier full/empty pairs (no CTA barrier in the loop) and a transposing, coalesced epilogue.
 #include <algorithm>
 #include <cstring>
 #include <type_traits>
@@ -202,7 +204,6 @@ static_assert((SB_P & (SB_P - 1)) == 0 && SB_P >= 2 && SB_D * 4 <= 32 && SB_WARP
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
 #undef SB_ROWS_PARAMS
-constexpr int SB_SLOT_CHUNKS_MAX = sb_phys(SB_NCH_MAX) + 1;
 
 __device__ __forceinline__ void sb_cp_async16_s(unsigned sa, const void *gmem) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
@@ -241,7 +242,7 @@ struct SbArgs {
     int ndm, nblk, gslots;
     int slot_chunks;          // physical 16-byte chunks per staged channel
     int first;                // 1: store, 0: add into out
-    unsigned zero;            // always 0, opaque to the compiler (subband_rows.inc)
+    unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
 };
 
 typedef unsigned long long sb_u64;  // one aligned register pair = two fp32 accumulators (FADD2 operand)

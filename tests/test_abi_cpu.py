@@ -98,3 +98,21 @@ def test_subband_records_encode_exactly_the_shift_table(name):
     sb = plan.subbands()
     assert sb[0] == 0 and sb[-1] == CONFIGS[name].nchans and np.all(np.diff(sb) > 0)
     assert plan.verify_records() == 0
+
+
+def test_generated_channel_body_is_up_to_date():
+    """subband_rows.inc is committed generated code: it must equal what gen_subband_rows.py emits for
+    its default (= plan.h) tile constants, so that the file and its generator cannot drift apart."""
+    import importlib.util
+    import os
+    csrc = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_1111_6399_b200", "csrc")
+    spec = importlib.util.spec_from_file_location("gen_subband_rows", os.path.join(csrc, "gen_subband_rows.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    with open(os.path.join(csrc, "subband_rows.inc")) as f:
+        committed = f.read()
+    d, k, omax, odd = (int(x) for x in committed.splitlines()[0].split("gen_subband_rows.py")[1].split("-")[0].split())
+    assert committed == gen.generate(d, k, omax, odd)
+    with open(os.path.join(csrc, "plan.h")) as f:
+        plan_h = f.read()
+    assert f"#define SB_D_CFG {d}" in plan_h and f"#define SB_K_CFG {k}" in plan_h and f"#define SB_OMAX_CFG {omax}" in plan_h
