@@ -358,8 +358,44 @@ def run_c5_stream(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def run_paper_sweep(args):
+    """the paper's Fig. 4 regime (ndm = nchans) as a second workload; one
+    JSON line per point, with the paper's own axis ("execution time as percentage of real-time")."""
+    import torch
+
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import paper_sweep, synth
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product has no CPU path"
+    _, sm_max_mhz, _ = _peaks()
+    peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6 / 1e9
+    points = [(n, 200.0) for n in (250, 500, 1000, 2000, 4000)] + [(2000, dm) for dm in (50.0, 100.0, 400.0, 800.0)]
+    for nchans, max_dm in points:
+        cfg = paper_sweep(nchans, max_dm)
+        plan = P.Plan.from_config(cfg)
+        x, _ = synth.make_input(cfg, plan.shifts(), cfg.nsamp_out + plan.max_shift, device="cuda")
+        out = plan.alloc_out(cfg.nsamp_out)
+        for _ in range(args.warmup):
+            plan.execute(x, cfg.nsamp_out, out)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            plan.execute(x, cfg.nsamp_out, out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        adds = cfg.ndm * cfg.nchans * cfg.nsamp_out
+        print(json.dumps({"workload": cfg.name, "nchans": nchans, "ndm": cfg.ndm, "max_dm": max_dm, "nsamp_out": cfg.nsamp_out,
+                          "passes": plan.num_subbands(), "kernel": plan.kernel, "ms_per_step": ms,
+                          "pct_of_real_time": 100.0 * ms * 1e-3 / (cfg.nsamp_out * cfg.tsamp),
+                          "gadds_per_s": adds / ms / 1e6, "frac_of_add_peak": adds / ms / 1e6 / peak}), flush=True)
+        del x, out, plan
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--sweep", default=None, choices=["paper"])
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
@@ -374,7 +410,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     from paper_1111_6399_b200 import CONFIGS
     cfg = CONFIGS[args.config]
-    if args.impl == "reference":
+    if args.sweep:
+        run_paper_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     elif args.config == "c5":
         run_c5_stream(args, cfg)

@@ -92,3 +92,13 @@ def shrink(cfg: SurveyConfig, nchans=None, nsamp_out=None, ndm_stride: int = 1,
     if out is not cfg:
         out = replace(out, name=cfg.name + "_shrunk")
     return out
+
+
+def paper_sweep(nchans: int, max_dm: float = 200.0, ndm: int | None = None, nsamp_out: int = 65536) -> SurveyConfig:
+    """The paper's own experiment regime (Fig. 4): ``ndm = nchans`` equally spaced
+    trials up to ``max_dm`` ("to ensure that we do not sub-sample the data"); left panel sweeps
+    nchans at max DM 200, right panel sweeps max DM at nchans = ndm = 2000. The paper gives neither
+    band nor sampling time for these runs: c2's LOFAR-like band and tsamp are used."""
+    ndm = nchans if ndm is None else ndm
+    return SurveyConfig(f"paper_nchan{nchans}_ndm{ndm}_dm{max_dm:g}", nchans, 159.0, -32.0 / nchans, 327.68e-6, nsamp_out,
+                        ((0.0, max_dm / max(ndm - 1, 1), ndm),), "u8", 128.0, 16.0, 20.0, 3, SEED0 + 100 + nchans)

@@ -9,7 +9,7 @@ import pytest
 import torch
 
 import paper_1111_6399_b200 as P
-from paper_1111_6399_b200 import CONFIGS, shrink
+from paper_1111_6399_b200 import CONFIGS, paper_sweep, shrink
 from paper_1111_6399_b200.configs import SurveyConfig
 
 from _util import assert_matches_oracle, make_case, oracle_table, oracle_rows, run_gpu, spread_rows
@@ -37,6 +37,7 @@ SMALL = {
     "c3s": shrink(CONFIGS["c3"], nchans=300, nsamp_out=4500, ndm_stride=31),
     "c4s": shrink(CONFIGS["c4"], nchans=257, nsamp_out=3100, ndm_stride=29),
     "c5s": shrink(CONFIGS["c5"], nchans=128, nsamp_out=2049, ndm_stride=5),
+    "paper": paper_sweep(250, 200.0, nsamp_out=3000),                     # PAPER.md:56-58 regime, ndm = nchans
     "fine": SurveyConfig("fine_dm_u8", 200, 159.0, -32.0 / 200.0, 327.68e-6, 3000, ((0.0, 0.01, 333),),
                          "u8", 128.0, 16.0, 20.0, 2, 77),                  # paper regime: adjacent-DM delta <= 1
 }
