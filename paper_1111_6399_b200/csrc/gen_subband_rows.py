@@ -44,7 +44,9 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
     P = K // 4                                  # chunks per lane = pad period (one pad chunk per P)
     NCHUNK = (K + OMAX + 3) // 4
     NW, NV, NO = 2 * NCHUNK, 2 * NCHUNK - 1, OMAX + 1
-    assert D * 4 <= 32 and OMAX <= 15 and P % 2 == 0
+    assert D * 4 <= 32 and OMAX <= 15 and K % 4 == 0
+    if P % 2 == 1:
+        head = "linear"                         # odd chunk count per lane: the plain layout is conflict-free
 
     def acc(j, k):
         return "%%%d" % (j * K2 + k)
@@ -136,7 +138,11 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
                 out.append("mov.b64 v%d, {h%d, l%d};" % (i, i, i + 1))
         return out + goto_row(0)
 
-    if head == "brx":
+    if head == "linear":
+        for m in range(NCHUNK):
+            L.append("ld.shared.v2.b64 {w%d, w%d}, [%s+%d];" % (2 * m, 2 * m + 1, SA, 16 * m))
+        L += after_loads()
+    elif head == "brx":
         # one jump on the pad phase ar into P copies of the loads with immediate offsets
         L.append("brx.idx.uni %s, TA;" % AR)
         for r in range(P):
@@ -176,7 +182,7 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
 
 if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
-    D, K, OMAX = a[:3] if len(a) >= 3 else (3, 32, 12)
+    D, K, OMAX = a[:3] if len(a) >= 3 else (3, 28, 12)
     sc = a[3] if len(a) > 3 else 2
     disp = {0: "tree", 1: "brx", 2: "ttree"}[a[4] if len(a) > 4 else 0]
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")

@@ -21,7 +21,7 @@ struct TiledGeom {
 // CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
 #ifndef SB_D_CFG
 #define SB_D_CFG 3
-#define SB_K_CFG 32
+#define SB_K_CFG 28
 #define SB_OMAX_CFG 12
 #endif
 #ifndef SB_WARPS_CFG

@@ -200,8 +200,12 @@ static_assert(SB_STAGES >= 4, "ring depth: prefetch distance SB_STAGES - 3 >= 1"
 static_assert(SB_CB <= SB_WARPS, "staging maps one warp to one channel of a stage");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
-__host__ __device__ constexpr int sb_phys(int chunk) { return chunk + chunk / SB_P; }  // 1 pad chunk per SB_P
-static_assert((SB_P & (SB_P - 1)) == 0 && SB_P >= 2 && SB_D * 4 <= 32 && SB_WARPS % 2 == 0, "tile constants");
+// Staged layout: lanes are SB_P chunks apart. Odd SB_P: the plain layout is already conflict-free for
+// LDS.128 (8 consecutive lanes hit 8 different 16-byte bank groups) and a channel's window is ONE
+// contiguous TMA bulk copy. Even SB_P: one pad chunk per SB_P chunks, copied with 16-byte cp.async.
+constexpr bool SB_PADDED = (SB_P % 2) == 0;
+__host__ __device__ constexpr int sb_phys(int chunk) { return SB_PADDED ? chunk + chunk / SB_P : chunk; }
+static_assert((!SB_PADDED || (SB_P & (SB_P - 1)) == 0) && SB_P >= 2 && SB_K % 4 == 0 && SB_D * 4 <= 32 && SB_WARPS % 2 == 0, "tile constants");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
 #undef SB_ROWS_PARAMS
@@ -214,6 +218,14 @@ __device__ __forceinline__ void sb_cp_async16_zs(unsigned sa, const void *gmem, 
 }
 __device__ __forceinline__ void sb_mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+// TMA bulk copy global -> shared (SASS UBLKCP); completion is counted in bytes on `bar`
+__device__ __forceinline__ void sb_bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void sb_mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void sb_mbar_arrive(unsigned bar) {
     asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
@@ -264,7 +276,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned stage_bytes = SB_CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
     uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
-    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 16u * (SB_P + 1) * lane;  // sb_phys(SB_P * lane)
+    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 16u * sb_phys(SB_P * lane);
     const unsigned zero = A.zero;
 
     sb_u64 acc[SB_D][SB_K / 2];
@@ -290,7 +302,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         return make_int2(0, 0);
     };
     int2 mt = load_meta(0);
-    auto issue = [&](int stage) {
+    auto issue = [&](int stage, unsigned full_bar) {
         const int c = A.c_begin + stage * SB_CB + warp;
         const int2 mt_cur = mt;
         mt = load_meta(stage + 1);
@@ -299,7 +311,13 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
             const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * sb_phys(lane);
             const float *src = in + e0 + 4 * lane;
-            if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
+            if (!SB_PADDED && e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
+                // plain layout, interior window: the whole window is one TMA bulk copy issued by one lane
+                if (lane == 0) {
+                    sb_mbar_expect_tx(full_bar, 16u * (unsigned)mt_cur.y);
+                    sb_bulk_g2s(sdata_base + buf * stage_bytes + warp * slot_bytes, in + e0, 16u * (unsigned)mt_cur.y, full_bar);
+                }
+            } else if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
 #pragma unroll
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it)
                     if (lane + 32 * it < mt_cur.y) sb_cp_async16_s(dst + 16u * sb_phys(32) * it, src + 128 * it);
@@ -335,13 +353,13 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     }
     __syncthreads();
 #pragma unroll
-    for (int st = 0; st < SB_DIST; ++st) { issue(st); sb_mbar_arrive_cp_async(bar_full + 8u * (st % SB_STAGES)); }
+    for (int st = 0; st < SB_DIST; ++st) { issue(st, bar_full + 8u * (st % SB_STAGES)); sb_mbar_arrive_cp_async(bar_full + 8u * (st % SB_STAGES)); }
     for (int stage = 0; stage < nstages; ++stage) {
         const int pst = stage + SB_DIST;
         if (pst < nstages) {
             const int pb = pst % SB_STAGES;
             if (pst >= SB_STAGES) sb_mbar_wait(bar_empty + 8u * pb, (unsigned)((pst / SB_STAGES - 1) & 1));
-            issue(pst);
+            issue(pst, bar_full + 8u * pb);
             sb_mbar_arrive_cp_async(bar_full + 8u * pb);
         } else {
             mt = make_int2(0, 0);
@@ -357,8 +375,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const uint2 rec = rec_next;                    // warp-uniform: x = SB_D 4-bit o_j, y = chunk base a
             rec_next = recp[min(ch + 1, SB_CB - 1) * SB_WARPS];
             const unsigned obits = rec.x;
-            const unsigned ar = rec.y & (unsigned)(SB_P - 1);
-            const unsigned sa = slot_u32 + ((rec.y + rec.y / SB_P) << 4);
+            const unsigned ar = SB_PADDED ? rec.y & (unsigned)(SB_P - 1) : 0u;
+            const unsigned sa = slot_u32 + ((unsigned)sb_phys((int)rec.y) << 4);
 #include "subband_rows.inc"
         }
         __syncwarp();
