@@ -81,8 +81,11 @@ int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1_mhz, doubl
  *          nsamp_out + dedisp_plan_max_shift(plan)); channel 0 = fch1 (highest frequency).
  *   d_out: [ndm][nsamp_out], row stride nsamp_out; int32 for DEDISP_U8 input (exact), float32 for
  *          DEDISP_F16 / DEDISP_F32 input (fp32 accumulation; summation order unspecified).
- * Allocates nothing. May be called repeatedly; concurrent calls on different streams are allowed
- * (the plan is read-only after create / set_kernel). EINVAL: NULLs, nsamp_out < 1. */
+ * May be called repeatedly. With DEDISP_F32 input whose base and row pitch are 16-byte aligned the
+ * call allocates nothing and the plan is read-only, so concurrent calls on different streams are
+ * allowed. With DEDISP_U8 / DEDISP_F16 input (or unaligned rows) the SUBBAND kernel first converts
+ * the input into a plan-owned fp32 scratch copy (grown on demand with cudaMalloc, freed at destroy):
+ * calls on one plan must then be ordered on one stream. EINVAL: NULLs, nsamp_out < 1. */
 int dedisp_execute(dedisp_plan *plan, const void *d_in, long long nsamp_out, void *d_out,
                    void *stream);
 
