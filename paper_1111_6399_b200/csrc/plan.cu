@@ -146,9 +146,40 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host output scratch");
         p->host_out_bytes = out_bytes;
     }
-    e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
+    // SUBBAND on aligned fp32 rows reads only the channels of its own sub-band in pass g: copy the
+    // sub-bands in pass order on a second stream and let pass g start as soon as its rows have landed,
+    // so that most of the H2D transfer hides under the earlier passes.
+    const bool overlap = resolve_kernel(p) == DEDISP_KERNEL_SUBBAND && p->dtype == DEDISP_F32 && (nsamp_in & 3) == 0 &&
+                         p->sb.passes.size() > 1;
+    if (overlap) {
+        if (!p->host_copy_st) {
+            e = cudaStreamCreateWithFlags(&p->host_copy_st, cudaStreamNonBlocking);
+            if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host copy stream");
+        }
+        while (p->host_pass_ready.size() < p->sb.passes.size()) {
+            cudaEvent_t ev;
+            e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+            if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host event");
+            p->host_pass_ready.push_back(ev);
+        }
+        cudaEvent_t start = p->host_pass_ready[0];           // order the copy stream after the caller's stream
+        e = cudaEventRecord(start, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_copy_st, start, 0);
+        const size_t row_bytes = (size_t)nsamp_in * sizeof(float);
+        for (size_t g = 0; g < p->sb.passes.size() && e == cudaSuccess; ++g) {
+            const SubbandPass &ps = p->sb.passes[g];
+            e = cudaMemcpyAsync((char *)p->d_host_in + ps.c_begin * row_bytes, (const char *)h_in + ps.c_begin * row_bytes,
+                                (size_t)(ps.c_end - ps.c_begin) * row_bytes, cudaMemcpyHostToDevice, p->host_copy_st);
+            if (e == cudaSuccess) e = cudaEventRecord(p->host_pass_ready[g], p->host_copy_st);
+        }
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
+        p->pass_ready = p->host_pass_ready.data();
+    } else {
+        e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
+    }
     const int rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+    p->pass_ready = nullptr;
     if (rc != DEDISP_OK) return rc;
     e = cudaMemcpyAsync(h_out, p->d_host_out, out_bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -161,6 +192,8 @@ int dedisp_plan_destroy(dedisp_plan *p) {
     if (p->d_shifts) cudaFree(p->d_shifts);
     if (p->d_host_in) cudaFree(p->d_host_in);
     if (p->d_host_out) cudaFree(p->d_host_out);
+    for (cudaEvent_t ev : p->host_pass_ready) cudaEventDestroy(ev);
+    if (p->host_copy_st) cudaStreamDestroy(p->host_copy_st);
     subband_free(p);
     delete p;
     return DEDISP_OK;

@@ -82,6 +82,10 @@ struct dedisp_plan {
     // scratch of dedisp_execute_host (grown on demand, freed at destroy)
     void *d_host_in = nullptr, *d_host_out = nullptr;
     size_t host_in_bytes = 0, host_out_bytes = 0;
+    // dedisp_execute_host overlap: a copy stream and one "rows of pass g are on the device" event per pass
+    cudaStream_t host_copy_st = nullptr;
+    std::vector<cudaEvent_t> host_pass_ready;
+    const cudaEvent_t *pass_ready = nullptr;  // set only for the duration of one dedisp_execute_host call
     // fp32 staging copy of the input for the SUBBAND kernel (u8/f16 input, or rows not 16-B aligned)
     float *d_conv = nullptr;
     size_t conv_bytes = 0;

@@ -545,6 +545,10 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         A.first = g == 0;
         const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
         dim3 grid((unsigned)(ntiles * sb.nblk), 1, (unsigned)b.n);
+        if (p->pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
+            e = cudaStreamWaitEvent(st, p->pass_ready[g], 0);
+            if (e != cudaSuccess) return e;
+        }
         kern<<<grid, SB_THREADS, smem, st>>>(A);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
