@@ -1,5 +1,6 @@
 // plan.cu — subsystem (1): the C ABI of include/dedisp.h (plan create / execute / destroy and
 // inspection). Host logic only; kernels live in kernels_tiled.cu and subband.cu.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -178,7 +179,40 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
     }
-    const int rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+    int rc = DEDISP_OK;
+    if (overlap && p->sb.nblk >= 4) {
+        // ... and run the passes slab by slab over the DM blocks, so that the D2H copy of a finished
+        // slab of out rows overlaps the passes of the next one
+        constexpr int NSLAB = 4;
+        if (!p->host_d2h_st) e = cudaStreamCreateWithFlags(&p->host_d2h_st, cudaStreamNonBlocking);
+        while (e == cudaSuccess && p->host_slab_done.size() < NSLAB) {
+            cudaEvent_t ev;
+            e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+            if (e == cudaSuccess) p->host_slab_done.push_back(ev);
+        }
+        if (e != cudaSuccess) { p->pass_ready = nullptr; return fail_cuda(p, e, "dedisp_execute_host slabs"); }
+        for (int sl = 0; sl < NSLAB && rc == DEDISP_OK; ++sl) {
+            p->sb_blk_begin = (int)((long long)p->sb.nblk * sl / NSLAB);
+            p->sb_blk_end = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
+            rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+            if (rc != DEDISP_OK) break;
+            const long long d0 = std::min<long long>(p->ndm, (long long)p->sb_blk_begin * SB_ROWS);
+            const long long d1 = std::min<long long>(p->ndm, (long long)p->sb_blk_end * SB_ROWS);
+            e = cudaEventRecord(p->host_slab_done[sl], st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_d2h_st, p->host_slab_done[sl], 0);
+            if (e == cudaSuccess && d1 > d0)
+                e = cudaMemcpyAsync((char *)h_out + d0 * nsamp_out * 4, (char *)p->d_host_out + d0 * nsamp_out * 4,
+                                    (size_t)(d1 - d0) * nsamp_out * 4, cudaMemcpyDeviceToHost, p->host_d2h_st);
+            if (e != cudaSuccess) rc = fail_cuda(p, e, "dedisp_execute_host slab D2H");
+        }
+        p->sb_blk_begin = 0; p->sb_blk_end = -1; p->pass_ready = nullptr;
+        if (rc != DEDISP_OK) return rc;
+        e = cudaStreamSynchronize(p->host_d2h_st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host D2H");
+        return DEDISP_OK;
+    }
+    rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
     p->pass_ready = nullptr;
     if (rc != DEDISP_OK) return rc;
     e = cudaMemcpyAsync(h_out, p->d_host_out, out_bytes, cudaMemcpyDeviceToHost, st);
@@ -194,6 +228,8 @@ int dedisp_plan_destroy(dedisp_plan *p) {
     if (p->d_host_out) cudaFree(p->d_host_out);
     for (cudaEvent_t ev : p->host_pass_ready) cudaEventDestroy(ev);
     if (p->host_copy_st) cudaStreamDestroy(p->host_copy_st);
+    for (cudaEvent_t ev : p->host_slab_done) cudaEventDestroy(ev);
+    if (p->host_d2h_st) cudaStreamDestroy(p->host_d2h_st);
     subband_free(p);
     delete p;
     return DEDISP_OK;

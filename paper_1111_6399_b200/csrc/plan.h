@@ -86,6 +86,9 @@ struct dedisp_plan {
     cudaStream_t host_copy_st = nullptr;
     std::vector<cudaEvent_t> host_pass_ready;
     const cudaEvent_t *pass_ready = nullptr;  // set only for the duration of one dedisp_execute_host call
+    int sb_blk_begin = 0, sb_blk_end = -1;    // DM-block range the next SUBBAND launch covers (-1: all); execute_host slabs
+    cudaStream_t host_d2h_st = nullptr;
+    std::vector<cudaEvent_t> host_slab_done;
     // fp32 staging copy of the input for the SUBBAND kernel (u8/f16 input, or rows not 16-B aligned)
     float *d_conv = nullptr;
     size_t conv_bytes = 0;

@@ -253,6 +253,7 @@ struct SbArgs {
     const int32_t *skew;      // this pass: [ndm]
     int c_begin, c_end;
     int ndm, nblk, gslots;
+    int blk0, nblk_run;       // this launch covers DM blocks [blk0, blk0 + nblk_run)
     int slot_chunks;          // physical 16-byte chunks per staged channel
     int first;                // 1: store, 0: add into out
     unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
@@ -264,8 +265,8 @@ template <typename OutT>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int blk = blockIdx.x % A.nblk;
-    const long long U0 = (long long)(blockIdx.x / A.nblk) * SB_T;
+    const int blk = A.blk0 + blockIdx.x % A.nblk_run;
+    const long long U0 = (long long)(blockIdx.x / A.nblk_run) * SB_T;
     const int d_first = blk * SB_ROWS;
     const int d_last = min(A.ndm, d_first + SB_ROWS) - 1;
     // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
@@ -530,6 +531,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.ndm = p->ndm;
     A.nblk = sb.nblk;
     A.gslots = sb.nblk * SB_WARPS;
+    A.blk0 = p->sb_blk_begin;
+    A.nblk_run = (p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end) - p->sb_blk_begin;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
     size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8 + 16 * SB_STAGES;
@@ -544,8 +547,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         A.c_end = ps.c_end;
         A.first = g == 0;
         const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
-        dim3 grid((unsigned)(ntiles * sb.nblk), 1, (unsigned)b.n);
-        if (p->pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
+        dim3 grid((unsigned)(ntiles * A.nblk_run), 1, (unsigned)b.n);
+        if (p->pass_ready && p->sb_blk_begin == 0) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
             e = cudaStreamWaitEvent(st, p->pass_ready[g], 0);
             if (e != cudaSuccess) return e;
         }
