@@ -109,8 +109,8 @@ int dedisp_execute_batched(dedisp_plan *plan, int nbeams, const void *d_in, long
  * asynchronous to the host and full speed). Copies the input to plan-owned device scratch (grown
  * on demand, freed at destroy), executes, copies the result back and SYNCHRONISES `stream` before
  * returning. For the SUBBAND kernel on 16-byte-aligned fp32 rows the input is copied per sub-band
- * pass on a plan-owned second stream, ordered after `stream`, and the result per DM slab on a third,
- * so both transfers overlap the passes. Not re-entrant per plan (the scratch is shared). */
+ * pass (smallest first) on a plan-owned second stream, ordered after `stream`, and the result per DM
+ * slab of the last pass on a third, so both transfers overlap the passes. Not re-entrant per plan (the scratch is shared). */
 int dedisp_execute_host(dedisp_plan *plan, const void *h_in, long long nsamp_out, void *h_out,
                         void *stream);
 

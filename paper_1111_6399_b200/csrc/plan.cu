@@ -167,7 +167,8 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         e = cudaEventRecord(start, st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_copy_st, start, 0);
         const size_t row_bytes = (size_t)nsamp_in * sizeof(float);
-        for (size_t g = 0; g < p->sb.passes.size() && e == cudaSuccess; ++g) {
+        for (size_t i = 0; i < p->sb.passes.size() && e == cudaSuccess; ++i) {
+            const size_t g = p->sb.passes.size() - 1 - i;     // last sub-band first: it has the fewest channels
             const SubbandPass &ps = p->sb.passes[g];
             e = cudaMemcpyAsync((char *)p->d_host_in + ps.c_begin * row_bytes, (const char *)h_in + ps.c_begin * row_bytes,
                                 (size_t)(ps.c_end - ps.c_begin) * row_bytes, cudaMemcpyHostToDevice, p->host_copy_st);
@@ -175,14 +176,15 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         }
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
         p->pass_ready = p->host_pass_ready.data();
+        p->sb_reverse = true;
     } else {
         e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
     }
     int rc = DEDISP_OK;
     if (overlap && p->sb.nblk >= 4) {
-        // ... and run the passes slab by slab over the DM blocks, so that the D2H copy of a finished
-        // slab of out rows overlaps the passes of the next one
+        // ... and run the LAST pass slab by slab over the DM blocks, so that the D2H copy of a finished
+        // slab of out rows overlaps the rest of that pass
         constexpr int NSLAB = 4;
         if (!p->host_d2h_st) e = cudaStreamCreateWithFlags(&p->host_d2h_st, cudaStreamNonBlocking);
         while (e == cudaSuccess && p->host_slab_done.size() < NSLAB) {
@@ -191,6 +193,11 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
             if (e == cudaSuccess) p->host_slab_done.push_back(ev);
         }
         if (e != cudaSuccess) { p->pass_ready = nullptr; return fail_cuda(p, e, "dedisp_execute_host slabs"); }
+        // all passes but the last over the whole grid, then the last pass slab by slab
+        const int npass = (int)p->sb.passes.size();
+        p->sb_pass_lo = 0; p->sb_pass_hi = npass - 1;
+        rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+        p->sb_pass_lo = npass - 1; p->sb_pass_hi = npass;
         for (int sl = 0; sl < NSLAB && rc == DEDISP_OK; ++sl) {
             p->sb_blk_begin = (int)((long long)p->sb.nblk * sl / NSLAB);
             p->sb_blk_end = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
@@ -205,7 +212,8 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
                                     (size_t)(d1 - d0) * nsamp_out * 4, cudaMemcpyDeviceToHost, p->host_d2h_st);
             if (e != cudaSuccess) rc = fail_cuda(p, e, "dedisp_execute_host slab D2H");
         }
-        p->sb_blk_begin = 0; p->sb_blk_end = -1; p->pass_ready = nullptr;
+        p->sb_pass_lo = 0; p->sb_pass_hi = -1;
+        p->sb_blk_begin = 0; p->sb_blk_end = -1; p->pass_ready = nullptr; p->sb_reverse = false;
         if (rc != DEDISP_OK) return rc;
         e = cudaStreamSynchronize(p->host_d2h_st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -214,6 +222,7 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
     }
     rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
     p->pass_ready = nullptr;
+    p->sb_reverse = false;
     if (rc != DEDISP_OK) return rc;
     e = cudaMemcpyAsync(h_out, p->d_host_out, out_bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);

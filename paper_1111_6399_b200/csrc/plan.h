@@ -86,6 +86,8 @@ struct dedisp_plan {
     cudaStream_t host_copy_st = nullptr;
     std::vector<cudaEvent_t> host_pass_ready;
     const cudaEvent_t *pass_ready = nullptr;  // set only for the duration of one dedisp_execute_host call
+    bool sb_reverse = false;                  // run the passes last sub-band first (execute_host: smallest H2D first)
+    int sb_pass_lo = 0, sb_pass_hi = -1;      // launch-order range of passes the next SUBBAND launch runs (-1: all)
     int sb_blk_begin = 0, sb_blk_end = -1;    // DM-block range the next SUBBAND launch covers (-1: all); execute_host slabs
     cudaStream_t host_d2h_st = nullptr;
     std::vector<cudaEvent_t> host_slab_done;

@@ -540,15 +540,17 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    for (size_t g = 0; g < sb.passes.size(); ++g) {
+    const size_t pass_hi = p->sb_pass_hi < 0 ? sb.passes.size() : (size_t)p->sb_pass_hi;
+    for (size_t i = (size_t)p->sb_pass_lo; i < pass_hi; ++i) {
+        const size_t g = p->sb_reverse ? sb.passes.size() - 1 - i : i;   // any order: the first launched pass stores
         const SubbandPass &ps = sb.passes[g];
         A.skew = sb.d_skew + g * (size_t)p->ndm;
         A.c_begin = ps.c_begin;
         A.c_end = ps.c_end;
-        A.first = g == 0;
+        A.first = i == 0;
         const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
         dim3 grid((unsigned)(ntiles * A.nblk_run), 1, (unsigned)b.n);
-        if (p->pass_ready && p->sb_blk_begin == 0) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
+        if (p->pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
             e = cudaStreamWaitEvent(st, p->pass_ready[g], 0);
             if (e != cudaSuccess) return e;
         }
