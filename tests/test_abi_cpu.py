@@ -116,3 +116,18 @@ def test_generated_channel_body_is_up_to_date():
     with open(os.path.join(csrc, "plan.h")) as f:
         plan_h = f.read()
     assert f"#define SB_D_CFG {d}" in plan_h and f"#define SB_K_CFG {k}" in plan_h and f"#define SB_OMAX_CFG {omax}" in plan_h
+
+
+def test_kernel_selection_falls_back_when_subband_is_not_admitted():
+    """AUTO resolves to SUBBAND only when the plan admits it: u8 sums must stay exact in fp32
+    (nchans*255 < 2^24), otherwise the int32 TILED kernel is used; forcing SUBBAND is refused."""
+    import paper_1111_6399_b200 as P
+    ok = P.Plan(512, 1500.0, -0.5, 64e-6, [0.0, 1.0, 2.0, 3.0], "u8", host_only=True)
+    assert ok.kernel == P.KERNEL_SUBBAND and ok.num_subbands() >= 1 and ok.verify_records() == 0
+    big = P.Plan(70000, 1500.0, -0.01, 64e-6, [0.0, 1.0], "u8", host_only=True)   # 70000*255 > 2^24
+    assert big.kernel == P.KERNEL_TILED and big.num_subbands() == 0
+    with pytest.raises(P.DedispError) as ei:
+        big.set_kernel(P.KERNEL_SUBBAND)
+    assert ei.value.code == 4
+    f32 = P.Plan(70000, 1500.0, -0.01, 64e-6, [0.0, 1.0], "f32", host_only=True)   # no exactness bound for fp32
+    assert f32.kernel == P.KERNEL_SUBBAND
