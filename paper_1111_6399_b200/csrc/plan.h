@@ -19,22 +19,38 @@ struct TiledGeom {
 // SUBBAND kernel (subband.cu): exact sub-band re-skewed multi-pass with register-window reuse.
 // Thread tile = SB_D DM rows x SB_K consecutive samples; warp = one DM group (SB_D rows) x 32 lanes;
 // CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
+// Two generated channel bodies exist (gen_subband_rows.py): SB_JOINT = 1 dispatches ONCE per channel on
+// the joint offset pattern of the thread's rows (window in 8-byte pairs, offsets 0..SB_S+1); SB_JOINT = 0
+// dispatches per row (window in 16-byte chunks, offsets 0..SB_OMAX).
+#ifndef SB_JOINT_CFG
+#define SB_JOINT_CFG 1
+#endif
 #ifndef SB_D_CFG
 #define SB_D_CFG 3
+#if SB_JOINT_CFG
+#define SB_K_CFG 26
+#else
 #define SB_K_CFG 28
+#endif
 #define SB_OMAX_CFG 12
+#endif
+#ifndef SB_S_CFG
+#define SB_S_CFG 3
 #endif
 #ifndef SB_WARPS_CFG
 #define SB_WARPS_CFG 12
 #endif
+constexpr bool SB_JOINT = SB_JOINT_CFG != 0;
 constexpr int SB_D = SB_D_CFG;
 constexpr int SB_K = SB_K_CFG;
 constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
 constexpr int SB_WARPS = SB_WARPS_CFG; // DM groups per CTA (one warp each)
 constexpr int SB_ROWS = SB_D * SB_WARPS;
-constexpr int SB_OMAX = SB_OMAX_CFG;  // largest in-window offset a row may have (bodies 0..SB_OMAX)
-constexpr int SB_P = SB_K / 4;        // 16-byte chunks per lane = pad period of the staged layout
-constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;  // 16-byte chunks a thread loads per channel
+constexpr int SB_S = SB_S_CFG;        // joint: largest spread of the residual delay over a thread's rows
+constexpr int SB_OMAX = SB_JOINT ? SB_S + 1 : SB_OMAX_CFG;  // largest in-window offset a row may have
+constexpr int SB_P = SB_K / 4;        // per-row mode: 16-byte chunks per lane (pad period if even)
+constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;   // per-row mode: 16-byte chunks a thread loads per channel
+constexpr int SB_WPAIRS = (SB_K + SB_OMAX + 1) / 2;    // joint mode: 8-byte pairs a thread loads per channel
 #ifndef SB_CB_CFG
 #define SB_CB_CFG 8
 #endif
@@ -43,7 +59,8 @@ constexpr int SB_CB = SB_CB_CFG;      // channels per pipeline stage (one stagin
 #define SB_STAGES_CFG 4
 #endif
 constexpr int SB_STAGES = SB_STAGES_CFG;
-constexpr int SB_NCH_MAX = SB_P * 32 + 96;  // staged chunks per channel the slot can hold (logical)
+// staged 16-byte chunks per channel the slot can hold (logical), a multiple of 32
+constexpr int SB_NCH_MAX = SB_JOINT ? ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 * 32 : SB_P * 32 + 96;
 
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;
@@ -54,7 +71,8 @@ struct SubbandGeom {
     bool ok = false;
     std::vector<SubbandPass> passes;
     int ngroups = 0, nblk = 0;
-    // per (channel, group): bits 0..31 eight 4-bit offsets o_j, bits 32..47 chunk base a (subband.cu)
+    // per (channel, group): low word = SB_D 4-bit offsets o_j (per-row mode) or the joint pattern id
+    // (o_0*(S+2) + o_1)*(S+2) + ..., high word = window base a in 16-byte chunks / 8-byte pairs (subband.cu)
     std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]
     // per (channel, block): {window base r (multiple of 4, relative to u), chunks to stage}
     std::vector<int32_t> meta;        // [nchans][nblk][2]

@@ -57,24 +57,31 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
             int bmin = INT32_MAX;
             for (int w = 0; w < SB_WARPS; ++w) bmin = std::min(bmin, gmin[b * SB_WARPS + w]);
             const int rbase = floor4(bmin);
+            // window base of a group inside the block's staged region: 16-byte chunks (per-row mode) or
+            // 8-byte pairs (joint mode); what is left of the residual delays are the in-window offsets
+            constexpr int AUNIT = SB_JOINT ? 2 : 4;
             int amax = 0;
             for (int w = 0; w < SB_WARPS; ++w) {
                 const int q = b * SB_WARPS + w;
-                const int a = (gmin[q] - rbase) >> 2;
-                if (gmax[q] - rbase - 4 * a > SB_OMAX) return false;
+                const int a = (gmin[q] - rbase) / AUNIT;
+                if (gmax[q] - rbase - AUNIT * a > SB_OMAX) return false;
+                if (SB_JOINT && gmax[q] - gmin[q] > SB_S) return false;
                 amax = std::max(amax, a);
                 if (emit) {
                     uint64_t rec = (uint64_t)a << 32;
                     const int qq = std::min(q, ngroups - 1);
+                    uint32_t lo = 0;
                     for (int j = 0; j < SB_D; ++j) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
-                        const int o = (sc[d] - sref[d]) - rbase - 4 * a;
-                        rec |= (uint64_t)o << (4 * j);
+                        const int o = (sc[d] - sref[d]) - rbase - AUNIT * a;
+                        if (SB_JOINT) lo = lo * (SB_S + 2) + (uint32_t)o;   // pattern id, row 0 most significant
+                        else lo |= (uint32_t)o << (4 * j);
                     }
-                    p->sb.records[(size_t)c * gslots + q] = rec;
+                    p->sb.records[(size_t)c * gslots + q] = rec | lo;
                 }
             }
-            const int nch = amax + SB_P * 31 + SB_WCHUNKS;
+            // staged 16-byte chunks: the furthest lane of the furthest group must find its whole window
+            const int nch = SB_JOINT ? (2 * amax + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 : amax + SB_P * 31 + SB_WCHUNKS;
             if (nch > SB_NCH_MAX || amax > 0xffff) return false;
             if (emit) {
                 p->sb.meta[((size_t)c * nblk + b) * 2 + 0] = rbase;
@@ -176,11 +183,20 @@ long long subband_verify_records(const dedisp_plan *p) {
             for (int d = 0; d < ndm; ++d) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
                 const uint64_t rec = sb.records[(size_t)c * gslots + q];
-                const int a = (int)((rec >> 32) & 0xffff), o = (int)((rec >> (4 * j)) & 15);
+                const int a = (int)((rec >> 32) & 0xffff);
+                int o;
+                if (SB_JOINT) {
+                    uint32_t id = (uint32_t)rec;
+                    for (int jj = SB_D - 1; jj > j; --jj) id /= (SB_S + 2);
+                    o = (int)(id % (SB_S + 2));
+                } else {
+                    o = (int)((rec >> (4 * j)) & 15);
+                }
                 const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
                 const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
-                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 4 * a + o;
-                if (s != p->shifts[(size_t)c * ndm + d] || a + SB_P * 31 + SB_WCHUNKS > nch || (rbase & 3) || o > SB_OMAX) ++bad;
+                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + (SB_JOINT ? 2 : 4) * a + o;
+                const int need = SB_JOINT ? (2 * a + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 : a + SB_P * 31 + SB_WCHUNKS;
+                if (s != p->shifts[(size_t)c * ndm + d] || need > nch || (rbase & 3) || o > SB_OMAX) ++bad;
             }
         }
     }
@@ -203,9 +219,11 @@ static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 // Staged layout: lanes are SB_P chunks apart. Odd SB_P: the plain layout is already conflict-free for
 // LDS.128 (8 consecutive lanes hit 8 different 16-byte bank groups) and a channel's window is ONE
 // contiguous TMA bulk copy. Even SB_P: one pad chunk per SB_P chunks, copied with 16-byte cp.async.
-constexpr bool SB_PADDED = (SB_P % 2) == 0;
+constexpr bool SB_PADDED = !SB_JOINT && (SB_P % 2) == 0;
 __host__ __device__ constexpr int sb_phys(int chunk) { return SB_PADDED ? chunk + chunk / SB_P : chunk; }
-static_assert((!SB_PADDED || (SB_P & (SB_P - 1)) == 0) && SB_P >= 2 && SB_K % 4 == 0 && SB_D * 4 <= 32 && SB_WARPS % 2 == 0, "tile constants");
+static_assert(SB_JOINT || ((!SB_PADDED || (SB_P & (SB_P - 1)) == 0) && SB_P >= 2 && SB_K % 4 == 0 && SB_D * 4 <= 32), "tile constants");
+static_assert(!SB_JOINT || (SB_K % 2 == 0 && (SB_K / 2) % 2 == 1), "joint mode: K/2 odd (LDS.64 conflict-free in the plain layout)");
+static_assert(SB_WARPS % 2 == 0 && SB_NCH_MAX % 32 == 0, "tile constants");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
 #undef SB_ROWS_PARAMS
@@ -256,9 +274,11 @@ struct SbArgs {
     int blk0, nblk_run;       // this launch covers DM blocks [blk0, blk0 + nblk_run)
     int slot_chunks;          // physical 16-byte chunks per staged channel
     int first;                // 1: store, 0: add into out
+    int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
     unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
 };
 
+constexpr int SB_EP_PITCH = (SB_K / 2) % 2 == 1 ? SB_K + 4 : SB_K + 2;  // epilogue transpose: words per lane
 typedef unsigned long long sb_u64;  // one aligned register pair = two fp32 accumulators (FADD2 operand)
 
 template <typename OutT>
@@ -277,7 +297,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned stage_bytes = SB_CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
     uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
-    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 16u * sb_phys(SB_P * lane);
+    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + (SB_JOINT ? 4u * SB_K * lane : 16u * sb_phys(SB_P * lane));
     const unsigned zero = A.zero;
 
     sb_u64 acc[SB_D][SB_K / 2];
@@ -377,7 +397,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             rec_next = recp[min(ch + 1, SB_CB - 1) * SB_WARPS];
             const unsigned obits = rec.x;
             const unsigned ar = SB_PADDED ? rec.y & (unsigned)(SB_P - 1) : 0u;
-            const unsigned sa = slot_u32 + ((unsigned)sb_phys((int)rec.y) << 4);
+            const unsigned sa = slot_u32 + (SB_JOINT ? rec.y << 3 : (unsigned)sb_phys((int)rec.y) << 4);
+            (void)ar; (void)zero;
 #include "subband_rows.inc"
         }
         __syncwarp();
@@ -388,16 +409,13 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     // sectors per instruction. Transpose through the (now idle) ring: each warp parks its tile in its
     // own padded region and writes / read-modify-writes out[d][t] with lanes on consecutive samples.
     __syncthreads();
-    constexpr int EP_PITCH = SB_K + 4;                       // words per lane: 16-byte aligned, odd number of chunks
+    constexpr int EP_PITCH = SB_EP_PITCH;                    // words per lane: an odd number of 8-byte pairs
     float *ep = reinterpret_cast<float *>(sb_smem) + (size_t)warp * (SB_D * 32 * EP_PITCH);
 #pragma unroll
     for (int j = 0; j < SB_D; ++j)
 #pragma unroll
-        for (int k4 = 0; k4 < SB_K / 4; ++k4) {
-            const sb_u64 p0 = acc[j][2 * k4], p1 = acc[j][2 * k4 + 1];
-            *reinterpret_cast<uint4 *>(ep + (j * 32 + lane) * EP_PITCH + 4 * k4) =
-                make_uint4((unsigned)p0, (unsigned)(p0 >> 32), (unsigned)p1, (unsigned)(p1 >> 32));
-        }
+        for (int k2 = 0; k2 < SB_K / 2; ++k2)
+            *reinterpret_cast<sb_u64 *>(ep + (j * 32 + lane) * EP_PITCH + 2 * k2) = acc[j][k2];
     __syncwarp();
     OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
 #pragma unroll 1
@@ -407,20 +425,44 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         const long long t0 = U0 - (long long)__ldg(A.skew + d);
         OutT *orow = out + (size_t)d * A.out_stride;
         const float *erow = ep + j * 32 * EP_PITCH;
-#pragma unroll 8
-        for (int i = 0; i < SB_K; ++i) {
-            const int sidx = i * 32 + lane;                  // sample within the tile, lanes consecutive
-            const float v = erow[(sidx / SB_K) * EP_PITCH + (sidx % SB_K)];
+        auto E = [&](int sidx) { return erow[(sidx / SB_K) * EP_PITCH + (sidx % SB_K)]; };
+        auto put = [&](int sidx) {                           // one sample, bounds-checked
             const long long t = t0 + sidx;
             if (t >= 0 && t < A.nsamp_out) {
                 if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
-                    const int vi = __float2int_rn(v);
+                    const int vi = __float2int_rn(E(sidx));
                     orow[t] = A.first ? vi : orow[t] + vi;
                 } else {
-                    orow[t] = A.first ? v : orow[t] + v;
+                    if (A.first) orow[t] = E(sidx);
+                    else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + t), "f"(E(sidx)) : "memory");
                 }
             }
+        };
+        if constexpr (std::is_floating_point<OutT>::value) {
+            if (A.out_vec4) {
+                // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
+                // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
+                const int m = (int)((-t0) & 3);              // samples before the first aligned t
+                const int nv = (SB_T - m) / 4;
+                for (int v = lane; v < nv; v += 32) {
+                    const int sidx = m + 4 * v;
+                    const long long t = t0 + sidx;
+                    if (t >= 0 && t + 3 < A.nsamp_out) {
+                        const float x0 = E(sidx), x1 = E(sidx + 1), x2 = E(sidx + 2), x3 = E(sidx + 3);
+                        if (A.first) *reinterpret_cast<float4 *>(orow + t) = make_float4(x0, x1, x2, x3);
+                        else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
+                                          ::"l"(orow + t), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
+                    } else {
+                        put(sidx); put(sidx + 1); put(sidx + 2); put(sidx + 3);
+                    }
+                }
+                if (lane < m) put(lane);                                             // head
+                if (lane < SB_T - (m + 4 * nv)) put(m + 4 * nv + lane);              // tail
+                continue;
+            }
         }
+#pragma unroll 8
+        for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
     }
 }
 
@@ -437,6 +479,16 @@ __global__ void __launch_bounds__(256) dedisp_to_f32_kernel(const TIN *__restric
     if constexpr (std::is_same<TIN, __half>::value) v = __half2float(src[i]);
     else v = (float)src[i];
     dst[i] = v;
+}
+
+// u8 plans: the passes accumulate exact fp32 sums in place in the caller's int32 buffer (so that every
+// pass can use the vector reduction); this turns the finished rows into int32, in place.
+__global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__restrict__ out, long long out_stride, long long out_beam,
+                                                                          long long nsamp_out, int d0) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsamp_out) return;
+    int *pv = out + (size_t)blockIdx.z * out_beam + (size_t)(d0 + blockIdx.y) * out_stride + i;
+    *pv = __float2int_rn(__int_as_float(*pv));
 }
 
 }  // namespace
@@ -474,7 +526,7 @@ static bool sb_needs_staging_copy(const dedisp_plan *p, const void *d_in, long l
 
 int subband_launches(const dedisp_plan *p, int resolved_kernel) {
     if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
-    return (int)p->sb.passes.size() + (p->dtype != DEDISP_F32 ? 1 : 0);
+    return (int)p->sb.passes.size() + (p->dtype != DEDISP_F32 ? 1 : 0) + (p->dtype == DEDISP_U8 ? 1 : 0);
 }
 
 cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams) {
@@ -526,6 +578,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.out_stride = out_stride;
     A.out_beam = b.out_stride;
     A.nsamp_out = nsamp_out;
+    A.out_vec4 = ((uintptr_t)d_out & 15) == 0 && (out_stride & 3) == 0 && (b.n == 1 || (b.out_stride & 3) == 0);
     A.records = sb.d_records;
     A.meta = sb.d_meta;
     A.ndm = p->ndm;
@@ -536,8 +589,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
     size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8 + 16 * SB_STAGES;
-    smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * (SB_K + 4) * sizeof(float));  // epilogue transpose region
-    auto kern = p->dtype == DEDISP_U8 ? dedisp_subband_kernel<int> : dedisp_subband_kernel<float>;
+    smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * SB_EP_PITCH * sizeof(float));  // epilogue transpose region
+    auto kern = dedisp_subband_kernel<float>;   // u8 plans too: fp32 sums in place, converted after the last pass
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const size_t pass_hi = p->sb_pass_hi < 0 ? sb.passes.size() : (size_t)p->sb_pass_hi;
@@ -557,6 +610,15 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         kern<<<grid, SB_THREADS, smem, st>>>(A);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
+    }
+    if (p->dtype == DEDISP_U8 && pass_hi == sb.passes.size()) {   // last pass done for these rows
+        const int d0 = std::min(p->ndm, A.blk0 * SB_ROWS), d1 = std::min(p->ndm, (A.blk0 + A.nblk_run) * SB_ROWS);
+        for (int r0 = d0; r0 < d1; r0 += 32768) {   // grid.y <= 65535
+            dim3 grid((unsigned)((nsamp_out + 255) / 256), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
+            dedisp_f32_to_i32_inplace_kernel<<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
     }
     return cudaSuccess;
 }
