@@ -213,7 +213,11 @@ namespace {
 
 constexpr int SB_THREADS = SB_WARPS * 32;
 static_assert(SB_STAGES >= 4, "ring depth: prefetch distance SB_STAGES - 3 >= 1");
-static_assert(SB_CB <= SB_WARPS, "staging maps one warp to one channel of a stage");
+#ifndef SB_CB_MAX_CFG
+#define SB_CB_MAX_CFG SB_WARPS
+#endif
+constexpr int SB_CB_MAX = SB_CB_MAX_CFG;   // channels per stage are chosen at launch (as many as fit): warp w stages w, w + SB_WARPS
+static_assert(SB_CB <= SB_WARPS, "the smallest stage: one channel per staging warp");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
 // Staged layout: lanes are SB_P chunks apart. Odd SB_P: the plain layout is already conflict-free for
@@ -273,6 +277,7 @@ struct SbArgs {
     int ndm, nblk, gslots;
     int blk0, nblk_run;       // this launch covers DM blocks [blk0, blk0 + nblk_run)
     int slot_chunks;          // physical 16-byte chunks per staged channel
+    int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
     int first;                // 1: store, 0: add into out
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
     unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
@@ -294,7 +299,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 
     const float *in = A.in + (size_t)blockIdx.z * A.in_beam;
     const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
-    const unsigned stage_bytes = SB_CB * slot_bytes;
+    const int CB = A.cb;
+    const unsigned stage_bytes = CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
     uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
     const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + (SB_JOINT ? 4u * SB_K * lane : 16u * sb_phys(SB_P * lane));
@@ -307,7 +313,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         for (int k = 0; k < SB_K / 2; ++k) acc[j][k] = 0ull;
 
     const int nchan = A.c_end - A.c_begin;
-    const int nstages = (nchan + SB_CB - 1) / SB_CB;
+    const int nstages = (nchan + CB - 1) / CB;
 
     // Staging: warp w copies channel w of the stage (SB_CB == SB_WARPS); lane l copies logical chunks
     // l, l+32, ... into the padded layout (sb_phys(l + 32 it) = sb_phys(l) + sb_phys(32) it). All of a warp's
@@ -317,26 +323,30 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
     // meta (window base, chunk count) of the channel this warp stages next: loaded one stage ahead so
     // that its L2 latency never sits in front of the copies
-    auto load_meta = [&](int stage) -> int2 {
-        const int c = A.c_begin + stage * SB_CB + warp;
-        if (stage < nstages && warp < SB_CB && c < A.c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
+    auto load_meta = [&](int stage, int k) -> int2 {
+        const int cc = warp + k * SB_WARPS;
+        const int c = A.c_begin + stage * CB + cc;
+        if (stage < nstages && cc < CB && c < A.c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
         return make_int2(0, 0);
     };
-    int2 mt = load_meta(0);
+    int2 mt[2] = {load_meta(0, 0), load_meta(0, 1)};
     auto issue = [&](int stage, unsigned full_bar) {
-        const int c = A.c_begin + stage * SB_CB + warp;
-        const int2 mt_cur = mt;
-        mt = load_meta(stage + 1);
-        if (stage < nstages && warp < SB_CB && c < A.c_end) {
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+        const int cc = warp + k * SB_WARPS;
+        const int c = A.c_begin + stage * CB + cc;
+        const int2 mt_cur = mt[k];
+        mt[k] = load_meta(stage + 1, k);
+        if (stage < nstages && cc < CB && c < A.c_end) {
             const int buf = stage % SB_STAGES;
             const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
-            const unsigned dst = sdata_base + buf * stage_bytes + warp * slot_bytes + 16u * sb_phys(lane);
+            const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes + 16u * sb_phys(lane);
             const float *src = in + e0 + 4 * lane;
             if (!SB_PADDED && e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
                 // plain layout, interior window: the whole window is one TMA bulk copy issued by one lane
                 if (lane == 0) {
                     sb_mbar_expect_tx(full_bar, 16u * (unsigned)mt_cur.y);
-                    sb_bulk_g2s(sdata_base + buf * stage_bytes + warp * slot_bytes, in + e0, 16u * (unsigned)mt_cur.y, full_bar);
+                    sb_bulk_g2s(sdata_base + buf * stage_bytes + cc * slot_bytes, in + e0, 16u * (unsigned)mt_cur.y, full_bar);
                 }
             } else if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
 #pragma unroll
@@ -352,8 +362,9 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                 }
             }
             if (lane < SB_WARPS / 2)   // the SB_WARPS records of this channel: contiguous, 16-byte aligned
-                sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * SB_CB + warp) * SB_WARPS) + 16u * lane,
+                sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * CB + cc) * SB_WARPS) + 16u * lane,
                                 reinterpret_cast<const char *>(A.records + (size_t)c * A.gslots + blk * SB_WARPS) + 16 * lane);
+        }
         }
     };
 
@@ -366,7 +377,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 #define SB_DIST_CFG (SB_STAGES - 3)
 #endif
     constexpr int SB_DIST = SB_DIST_CFG;
-    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + SB_STAGES * SB_CB * SB_WARPS);
+    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + SB_STAGES * CB * SB_WARPS);
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
     if (tid == 0) {
 #pragma unroll
@@ -382,19 +393,17 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             if (pst >= SB_STAGES) sb_mbar_wait(bar_empty + 8u * pb, (unsigned)((pst / SB_STAGES - 1) & 1));
             issue(pst, bar_full + 8u * pb);
             sb_mbar_arrive_cp_async(bar_full + 8u * pb);
-        } else {
-            mt = make_int2(0, 0);
         }
         sb_mbar_wait(bar_full + 8u * (stage % SB_STAGES), (unsigned)((stage / SB_STAGES) & 1));
         const int buf = stage % SB_STAGES;
-        const int nch = min(SB_CB, nchan - stage * SB_CB);
-        const uint2 *recp = srec + (buf * SB_CB) * SB_WARPS + warp;
+        const int nch = min(CB, nchan - stage * CB);
+        const uint2 *recp = srec + (buf * CB) * SB_WARPS + warp;
         unsigned slot_u32 = sdata_u32 + buf * stage_bytes;
         uint2 rec_next = *recp;                            // record of channel ch+1 is fetched one channel ahead
 #pragma unroll 1
         for (int ch = 0; ch < nch; ++ch, slot_u32 += slot_bytes) {
             const uint2 rec = rec_next;                    // warp-uniform: x = SB_D 4-bit o_j, y = chunk base a
-            rec_next = recp[min(ch + 1, SB_CB - 1) * SB_WARPS];
+            rec_next = recp[min(ch + 1, CB - 1) * SB_WARPS];
             const unsigned obits = rec.x;
             const unsigned ar = SB_PADDED ? rec.y & (unsigned)(SB_P - 1) : 0u;
             const unsigned sa = slot_u32 + (SB_JOINT ? rec.y << 3 : (unsigned)sb_phys((int)rec.y) << 4);
@@ -588,7 +597,12 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.nblk_run = (p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end) - p->sb_blk_begin;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
-    size_t smem = (size_t)SB_STAGES * SB_CB * A.slot_chunks * 16 + (size_t)SB_STAGES * SB_CB * SB_WARPS * 8 + 16 * SB_STAGES;
+    // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
+    auto ring_bytes = [&](int cb) { return (size_t)SB_STAGES * cb * A.slot_chunks * 16 + (size_t)SB_STAGES * cb * SB_WARPS * 8 + 16 * SB_STAGES; };
+    A.cb = SB_CB;
+    for (int cb = SB_CB_MAX; cb > SB_CB; cb -= 2)
+        if (ring_bytes(cb) <= 227u * 1024u) { A.cb = cb; break; }
+    size_t smem = ring_bytes(A.cb);
     smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * SB_EP_PITCH * sizeof(float));  // epilogue transpose region
     auto kern = dedisp_subband_kernel<float>;   // u8 plans too: fp32 sums in place, converted after the last pass
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
