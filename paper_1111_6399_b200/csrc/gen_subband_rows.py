@@ -180,66 +180,79 @@ def generate(D, K, OMAX, shifted_copy, dispatch="tree", head="arith"):
     return head + params + "asm volatile(\n%s\n    : %s\n    : %s\n    : \"memory\");\n#endif\n" % (text, outs, ins)
 
 
-def generate_joint(D, K, S):
-    """SB_JOINT = 1: ONE dispatch per channel on the joint offset pattern of all D rows.
+def generate_joint(D, K, S, G=None):
+    """SB_JOINT = 1: one dispatch per GROUP of G rows (default G = D: ONE per channel) on the joint
+    offset pattern of the group's rows.
 
     The window is loaded as 8-byte pairs (LDS.64; with K/2 odd the plain layout is conflict-free), so
     its base is 2-word aligned and the smallest in-window offset is 0 or 1; the sub-bands are cut so
-    that the offsets of a thread's rows spread by <= S.  The pattern id (o_0*(S+2) + o_1)*(S+2) + ...
-    indexes a jump table with one body per valid tuple (min in {0,1}, max - min <= S) holding all D
-    rows' adds with static register operands: 1 indirect branch per D*K adds instead of D branch trees.
-    Only the few patterns that adjacent row groups and neighbouring channels actually produce are hot
-    in the instruction cache (measured on c3: 16-18 of 122 for S = 4), so the table may be large."""
+    that the offsets of a thread's rows spread by <= S.  A group's pattern id (o_a*(S+2) + o_b)*(S+2)...
+    (8 bits per group in the record) indexes a jump table with one body per possible tuple holding the
+    group's adds with static register operands; the body ends with the jump of the next group.  Only
+    the few patterns that adjacent row groups and neighbouring channels actually produce are hot in the
+    instruction cache (measured on c3: 16-18 of 122 for D = G = 3, S = 4), so the tables may be large."""
     import itertools
+    G = D if G is None else G
+    assert D % G == 0 and (S + 2) ** G <= 256
     K2, OM = K // 2, S + 1
     NP = (K + OM + 1) // 2
+    NG = D // G
     assert K % 2 == 0 and K2 % 2 == 1, "K/2 must be odd: LDS.64 lanes K/2 pairs apart are then conflict-free"
 
     def acc(j, k):
         return "%%%d" % (j * K2 + k)
 
     SA, PID = "%%%d" % (D * K2), "%%%d" % (D * K2 + 1)
-    L = ["{", ".reg .f32 al, ah, lf<%d>, hf<%d>;" % (NP, NP), ".reg .b64 w<%d>;" % NP]
-    tuples = list(itertools.product(range(S + 2), repeat=D))          # id order: row 0 most significant
-    valid = [min(t) <= 1 and max(t) - min(t) <= S for t in tuples]
-    L.append("TP: .branchtargets %s;" % ", ".join(("B%d" % i) if v else "DONE" for i, v in enumerate(valid)))
+    L = ["{", ".reg .f32 al, ah, lf<%d>, hf<%d>;" % (NP, NP), ".reg .b64 w<%d>;" % NP, ".reg .b32 t<%d>;" % NG]
+    tuples = list(itertools.product(range(S + 2), repeat=G))           # id order: first row most significant
+    if NG == 1:   # the whole thread: min offset is 0 or 1 by construction
+        valid = [min(t) <= 1 and max(t) - min(t) <= S for t in tuples]
+    else:
+        valid = [max(t) - min(t) <= S for t in tuples]
+    for g in range(NG):
+        L.append("TP%d: .branchtargets %s;" % (g, ", ".join(("B%d_%d" % (g, i)) if v else "DONE" for i, v in enumerate(valid))))
     for m in range(NP):
         L.append("ld.shared.b64 w%d, [%s+%d];" % (m, SA, 8 * m))
+    for g in range(NG):
+        L.append("bfe.u32 t%d, %s, %d, 8;" % (g, PID, 8 * g))
     for m in range(NP):
         L.append("mov.b64 {lf%d, hf%d}, w%d;" % (m, m, m))
-    L.append("brx.idx.uni %s, TP;" % PID)
-    for i, (t, v) in enumerate(zip(tuples, valid)):
-        if not v:
-            continue
-        L.append("B%d:" % i)
-        for j, o in enumerate(t):
-            for k in range(K2):
-                m = (o >> 1) + k
-                if o & 1:   # odd offset: two scalar FADDs on the halves of the accumulator pair
-                    L += ["mov.b64 {al, ah}, %s;" % acc(j, k), "add.rn.f32 al, al, hf%d;" % m,
-                          "add.rn.f32 ah, ah, lf%d;" % (m + 1), "mov.b64 %s, {al, ah};" % acc(j, k)]
-                else:
-                    L.append("add.rn.f32x2 %s, %s, w%d;" % (acc(j, k), acc(j, k), m))
-        L.append("bra.uni DONE;")
+    L.append("brx.idx.uni t0, TP0;")
+    for g in range(NG):
+        for i, (t, v) in enumerate(zip(tuples, valid)):
+            if not v:
+                continue
+            L.append("B%d_%d:" % (g, i))
+            for jj, o in enumerate(t):
+                j = g * G + jj
+                for k in range(K2):
+                    m = (o >> 1) + k
+                    if o & 1:   # odd offset: two scalar FADDs on the halves of the accumulator pair
+                        L += ["mov.b64 {al, ah}, %s;" % acc(j, k), "add.rn.f32 al, al, hf%d;" % m,
+                              "add.rn.f32 ah, ah, lf%d;" % (m + 1), "mov.b64 %s, {al, ah};" % acc(j, k)]
+                    else:
+                        L.append("add.rn.f32x2 %s, %s, w%d;" % (acc(j, k), acc(j, k), m))
+            L.append("brx.idx.uni t%d, TP%d;" % (g + 1, g + 1) if g + 1 < NG else "bra.uni DONE;")
     L += ["DONE:", "}"]
     text = "\n".join('    "%s\\n"' % x for x in L)
     outs = ", ".join('"+l"(acc[%d][%d])' % (j, k) for j in range(D) for k in range(K2))
-    head = ("// GENERATED by gen_subband_rows.py joint %d %d %d - do not edit.\n"
-            "// One channel of the SUBBAND kernel, joint dispatch: %d LDS.64, one jump on the pattern id into %d bodies.\n"
-            % (D, K, S, NP, sum(valid)))
+    head = ("// GENERATED by gen_subband_rows.py joint %d %d %d %d - do not edit.\n"
+            "// One channel of the SUBBAND kernel, joint dispatch: %d LDS.64, %d jump(s) on a pattern id into %d bodies each.\n"
+            % (D, K, S, G, NP, NG, sum(valid)))
     params = ("#ifdef SB_ROWS_PARAMS\n"
-              "static_assert(SB_JOINT && SB_D == %d && SB_K == %d && SB_S == %d, \"regenerate subband_rows.inc (gen_subband_rows.py)\");\n"
-              "#else\n" % (D, K, S))
+              "static_assert(SB_JOINT && SB_D == %d && SB_K == %d && SB_S == %d && SB_G == %d, \"regenerate subband_rows.inc (gen_subband_rows.py)\");\n"
+              "#else\n" % (D, K, S, G))
     return head + params + "asm volatile(\n%s\n    : %s\n    : \"r\"(sa), \"r\"(obits)\n    : \"memory\");\n#endif\n" % (text, outs)
 
 
 if __name__ == "__main__" and (len(sys.argv) < 2 or sys.argv[1] == "joint"):
     a = [int(x) for x in sys.argv[2:]]
-    D, K, S = a[:3] if len(a) >= 3 else (3, 26, 3)
+    D, K, S = a[:3] if len(a) >= 3 else (4, 26, 4)
+    G = a[3] if len(a) > 3 else (2 if len(a) < 3 else D)
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:
-        f.write(generate_joint(D, K, S))
-    print(path, "joint", D, K, S)
+        f.write(generate_joint(D, K, S, G))
+    print(path, "joint", D, K, S, G)
 elif __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
     D, K, OMAX = a[:3] if len(a) >= 3 else (3, 28, 12)

@@ -26,7 +26,12 @@ struct TiledGeom {
 #define SB_JOINT_CFG 1
 #endif
 #ifndef SB_D_CFG
+#if SB_JOINT_CFG
+#define SB_D_CFG 4
+#define SB_G_CFG 2
+#else
 #define SB_D_CFG 3
+#endif
 #if SB_JOINT_CFG
 #define SB_K_CFG 26
 #else
@@ -35,7 +40,7 @@ struct TiledGeom {
 #define SB_OMAX_CFG 12
 #endif
 #ifndef SB_S_CFG
-#define SB_S_CFG 3
+#define SB_S_CFG 4
 #endif
 #ifndef SB_WARPS_CFG
 #define SB_WARPS_CFG 12
@@ -46,6 +51,10 @@ constexpr int SB_K = SB_K_CFG;
 constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
 constexpr int SB_WARPS = SB_WARPS_CFG; // DM groups per CTA (one warp each)
 constexpr int SB_ROWS = SB_D * SB_WARPS;
+#ifndef SB_G_CFG
+#define SB_G_CFG SB_D_CFG
+#endif
+constexpr int SB_G = SB_G_CFG;        // joint: rows per dispatch group (SB_D: one jump per channel)
 constexpr int SB_S = SB_S_CFG;        // joint: largest spread of the residual delay over a thread's rows
 constexpr int SB_OMAX = SB_JOINT ? SB_S + 1 : SB_OMAX_CFG;  // largest in-window offset a row may have
 constexpr int SB_P = SB_K / 4;        // per-row mode: 16-byte chunks per lane (pad period if even)

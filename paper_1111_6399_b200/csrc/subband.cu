@@ -74,8 +74,13 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
                     for (int j = 0; j < SB_D; ++j) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
                         const int o = (sc[d] - sref[d]) - rbase - AUNIT * a;
-                        if (SB_JOINT) lo = lo * (SB_S + 2) + (uint32_t)o;   // pattern id, row 0 most significant
-                        else lo |= (uint32_t)o << (4 * j);
+                        if (SB_JOINT) {   // 8 bits per dispatch group: pattern id, the group's first row most significant
+                            const int g = j / SB_G, sh = 8 * g;
+                            const uint32_t id = ((lo >> sh) & 255u) * (SB_S + 2) + (uint32_t)o;
+                            lo = (lo & ~(255u << sh)) | (id << sh);
+                        } else {
+                            lo |= (uint32_t)o << (4 * j);
+                        }
                     }
                     p->sb.records[(size_t)c * gslots + q] = rec | lo;
                 }
@@ -186,8 +191,8 @@ long long subband_verify_records(const dedisp_plan *p) {
                 const int a = (int)((rec >> 32) & 0xffff);
                 int o;
                 if (SB_JOINT) {
-                    uint32_t id = (uint32_t)rec;
-                    for (int jj = SB_D - 1; jj > j; --jj) id /= (SB_S + 2);
+                    uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
+                    for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
                     o = (int)(id % (SB_S + 2));
                 } else {
                     o = (int)((rec >> (4 * j)) & 15);

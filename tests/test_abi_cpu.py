@@ -115,10 +115,10 @@ def test_generated_channel_body_is_up_to_date():
     with open(os.path.join(csrc, "plan.h")) as f:
         plan_h = f.read()
     if tok[0] == "joint":
-        d, k, s = (int(x) for x in tok[1:4])
-        assert committed == gen.generate_joint(d, k, s)
+        d, k, s, g = (int(x) for x in tok[1:5])
+        assert committed == gen.generate_joint(d, k, s, g)
         assert "#define SB_JOINT_CFG 1" in plan_h and f"#define SB_D_CFG {d}" in plan_h
-        assert f"#define SB_K_CFG {k}" in plan_h and f"#define SB_S_CFG {s}" in plan_h
+        assert f"#define SB_K_CFG {k}" in plan_h and f"#define SB_S_CFG {s}" in plan_h and f"#define SB_G_CFG {g}" in plan_h
     else:
         d, k, omax, odd = (int(x) for x in tok[:4])
         assert committed == gen.generate(d, k, omax, odd)
