@@ -12,15 +12,17 @@
 // That only pays when adjacent trials' delays differ by a few samples. The survey configs' DM plans
 // are much coarser than the paper's (ndm = nchans), so the channels are split into sub-bands and
 // each sub-band is processed in the skewed time coordinate u = t + s(c_ref, d): the residual delay
-// r(c,d) = s(c,d) - s(c_ref,d) varies by <= SB_OMAX-3 samples across a thread's SB_D rows.
-// One kernel launch per sub-band ("pass"); pass 0 stores, later passes add into out.
+// r(c,d) = s(c,d) - s(c_ref,d) varies by <= SB_S samples across a thread's SB_D rows.
+// One kernel launch per sub-band ("pass"); the first pass stores, later passes add into out.
 //
-// Per channel a thread: its record (prefetched one channel ahead), SB_WCHUNKS LDS.128 of the window,
-// then for each of its SB_D rows a warp-uniform tree of direct branches on the row's offset o_j into
-// a body with static register operands (registers cannot be indexed dynamically): SB_K/2 FADD2 for
-// even o_j, SB_K scalar FADD for odd o_j. That body is generated inline PTX: see gen_subband_rows.py
-// for why and subband_rows.inc for the text. Around it: an SB_STAGES-deep cp.async ring handed over
-// with mbarrier full/empty pairs (no CTA barrier in the loop) and a transposing, coalesced epilogue.
+// Per channel a thread: its record (prefetched one channel ahead), SB_WPAIRS LDS.64 of the window,
+// then per group of SB_G rows ONE warp-uniform indirect branch on the group's joint offset pattern
+// into a body with static register operands (registers cannot be indexed dynamically): SB_K/2 FADD2
+// per row with an even offset, SB_K scalar FADD per row with an odd one. That body is generated
+// inline PTX: see gen_subband_rows.py for why and subband_rows.inc for the text (SB_JOINT_CFG=0
+// selects the older per-row dispatch). Around it: an SB_STAGES-deep ring filled by TMA bulk copies
+// and handed over with mbarrier full/empty pairs (no CTA barrier in the loop), and a transposing
+// epilogue that writes out with vector stores / red.global.add.v4.f32.
 #include <algorithm>
 #include <cstring>
 #include <type_traits>
