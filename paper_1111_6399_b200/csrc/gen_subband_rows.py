@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """Generates ``subband_rows.inc`` — the per-channel body of the SUBBAND kernel (subband.cu) as one
-inline-PTX statement.  ``python gen_subband_rows.py [D K OMAX [odd_mode [dispatch]]]`` after changing
-a tile constant; the generated file is committed so that the build needs nvcc only, and subband.cu
+inline-PTX statement.  ``python gen_subband_rows.py joint [D K S G]`` (the committed joint-pattern body,
+see generate_joint) or ``python gen_subband_rows.py D K OMAX [odd_mode [dispatch]]`` (the per-row body
+described below, SB_JOINT_CFG=0) after changing a tile constant; the generated file is committed so that the build needs nvcc only, and subband.cu
 static_asserts that its constants (plan.h) match the ones the file was generated for.
 
 Why PTX: a thread owns SB_D DM rows x SB_K consecutive samples and holds the union of its rows'
@@ -12,7 +13,7 @@ of SB_OMAX+1 bodies with static register operands.  Measured on c3 (profiles/r1_
   * a C++ ``switch`` is if-converted by nvcc into select chains (13 predicated moves per add): 9.5 %;
   * dispatch 1, "brx": threaded code, every body ends with the ``brx.idx`` of the next row (LDC from
     the jump table + BRX, ~88 cycles of warp latency per row): 15 %;
-  * dispatch 0, "tree" (committed): a binary tree of direct ``@q bra.uni`` on the four bits of o_j, the
+  * dispatch 0, "tree" (default of the per-row body): a binary tree of direct ``@q bra.uni`` on the four bits of o_j, the
     predicates set one body ahead; a taken direct branch costs ~12 cycles;
   * dispatch 2, "ttree": a private copy of the next row's tree in every body (no merge point, so no
     BSSY/BSYNC per row) — larger code, measured 1 % slower.
@@ -25,9 +26,12 @@ Adds are ``add.rn.f32x2`` (SASS FADD2: two fp32 adds per lane per issue slot).  
     costs 2*NCHUNK*2 registers and ALU-pipe time;
   * odd_mode 0: plain moves; ptxas sinks 2 IMAD.MOV per FADD2 into the odd bodies — they run on the
     fp32 pipe and steal its cycles;
-  * odd_mode 2 (committed): two scalar ``add.rn.f32`` on the halves of the accumulator pair — the same
+  * odd_mode 2 (default, also used by the joint body): two scalar ``add.rn.f32`` on the halves of the accumulator pair — the same
     fp32-pipe time as one FADD2, one more issue slot, no moves, no extra registers (this is what
     lets 3 warps per scheduler fit: 168 registers).
+
+The per-row body tops out at 35 % of the add peak on c3 because every row pays a branch tree; the
+joint body (generate_joint) dispatches once per group of rows and reaches 46 %.
 
 The window's pad phase (where in the padded shared-memory layout the lane's first chunk falls) is
 handled branch-free: chunk m sits at sa + 16*(m + m/P) + 16*[ar >= P - m%P].
