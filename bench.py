@@ -184,6 +184,8 @@ def run_ours(args, cfg):
     plan = P.Plan.from_config(cfg)                      # table build + upload: once per plan, not per step
     if args.kernel:
         plan.set_kernel({"naive": 1, "tiled": 2, "subband": 3}[args.kernel])
+    if args.merge_passes:
+        plan.set_pass_merge(True)
     nsamp_in = cfg.nsamp_out + plan.max_shift
     # each rank de-disperses its own beam (independent problems, no data-path collective): weak scaling
     x, _ = synth.make_input(cfg, plan.shifts(), nsamp_in, device="cuda", seed=beam_seed(cfg.seed, rank))
@@ -402,6 +404,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--kernel", default=None, choices=["naive", "tiled", "subband"])
+    ap.add_argument("--merge-passes", action="store_true", help="fp plans: all SUBBAND passes in one launch (not bit-reproducible)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-e2e", action="store_true")

@@ -124,6 +124,14 @@ int dedisp_plan_ndm(const dedisp_plan *plan);
 int dedisp_plan_get_shifts(const dedisp_plan *plan, int *h_out);
 /* Force a kernel (enum dedisp_kernel). EUNSUPPORTED if the plan does not admit it. */
 int dedisp_plan_set_kernel(dedisp_plan *plan, int kernel);
+/* SUBBAND pass merging. The SUBBAND kernel runs one launch per sub-band pass, each adding its partial
+ * sums into out in a fixed order (bit-reproducible results). With merging ON all passes run in ONE
+ * launch: out is zeroed and every pass adds with L2 reductions in whatever order the hardware
+ * schedules them. Integer-valued sums (DEDISP_U8 plans) are exact and therefore identical either way, so
+ * u8 plans merge on their own whenever it is faster (many short passes); for DEDISP_F16 / DEDISP_F32
+ * plans merging is OFF unless enabled here, and when ON the fp32 sums may differ in their last bits from run to run (still within the 1e-5 * sum|terms|
+ * bound). on = 0 / 1; EINVAL on NULL. */
+int dedisp_plan_set_pass_merge(dedisp_plan *plan, int on);
 /* The kernel dedisp_execute will launch for this plan (resolved, never AUTO). */
 int dedisp_plan_get_kernel(const dedisp_plan *plan);
 /* Sub-band layout of the SUBBAND kernel: number of passes G (0 if the plan has none) and, if

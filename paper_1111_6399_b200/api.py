@@ -29,7 +29,7 @@ SYMBOLS = (
     "dedisp_shift_table_host", "dedisp_plan_create", "dedisp_plan_create_ex", "dedisp_execute",
     "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
-    "dedisp_plan_get_kernel", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
+    "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
     "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_error_string",
     "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_sync",
     "dedisp_stream_destroy",
@@ -61,11 +61,12 @@ def lib() -> ctypes.CDLL:
         L.dedisp_plan_destroy.argtypes = [vp]
         L.dedisp_plan_max_shift.argtypes = [vp]
         L.dedisp_plan_max_shift.restype = c_ll
-        for name in ("dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_kernel", "dedisp_plan_num_subbands",
+        for name in ("dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands",
                      "dedisp_plan_launches_per_execute"):
             getattr(L, name).argtypes = [vp]
         L.dedisp_plan_get_shifts.argtypes = [vp, ip]
         L.dedisp_plan_set_kernel.argtypes = [vp, c_int]
+        L.dedisp_plan_set_pass_merge.argtypes = [vp, c_int]
         L.dedisp_plan_get_subbands.argtypes = [vp, ip]
         L.dedisp_plan_verify_records.argtypes = [vp]
         L.dedisp_plan_verify_records.restype = c_ll
@@ -136,6 +137,10 @@ class Plan:
 
     def set_kernel(self, kernel: int) -> None:
         self._check(lib().dedisp_plan_set_kernel(self._h, int(kernel)), "dedisp_plan_set_kernel")
+
+    def set_pass_merge(self, on: bool) -> None:
+        """``dedisp_plan_set_pass_merge``: all SUBBAND passes in one launch (fp sums then not bit-reproducible)."""
+        self._check(lib().dedisp_plan_set_pass_merge(self._h, int(bool(on))), "dedisp_plan_set_pass_merge")
 
     @property
     def kernel(self) -> int:

@@ -267,6 +267,12 @@ int dedisp_plan_set_kernel(dedisp_plan *p, int kernel) {
     return DEDISP_OK;
 }
 
+int dedisp_plan_set_pass_merge(dedisp_plan *p, int on) {
+    if (!p) return DEDISP_EINVAL;
+    p->merge_fp_passes = on != 0;
+    return DEDISP_OK;
+}
+
 int dedisp_plan_get_kernel(const dedisp_plan *p) { return p ? resolve_kernel(p) : -1; }
 
 int dedisp_plan_num_subbands(const dedisp_plan *p) {

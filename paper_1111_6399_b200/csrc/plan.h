@@ -89,6 +89,8 @@ struct SubbandGeom {
     uint64_t *d_records = nullptr;
     int32_t *d_meta = nullptr;
     int32_t *d_skew = nullptr;
+    int4 *d_ptab = nullptr;           // merged launch: per-pass {c_begin, c_end, pass, CTAs} for ptab_nsamp
+    long long ptab_nsamp = -1;
     int max_nch = 0;                  // largest staged chunk count (sizes the shared-memory slot)
 };
 
@@ -113,6 +115,7 @@ struct dedisp_plan {
     cudaStream_t host_copy_st = nullptr;
     std::vector<cudaEvent_t> host_pass_ready;
     const cudaEvent_t *pass_ready = nullptr;  // set only for the duration of one dedisp_execute_host call
+    bool merge_fp_passes = false;             // fp plans: run all passes in one launch (sums not bit-reproducible)
     bool sb_reverse = false;                  // run the passes last sub-band first (execute_host: smallest H2D first)
     int sb_pass_lo = 0, sb_pass_hi = -1;      // launch-order range of passes the next SUBBAND launch runs (-1: all)
     int sb_blk_begin = 0, sb_blk_end = -1;    // DM-block range the next SUBBAND launch covers (-1: all); execute_host slabs

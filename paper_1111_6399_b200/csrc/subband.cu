@@ -286,6 +286,7 @@ struct SbArgs {
     int slot_chunks;          // physical 16-byte chunks per staged channel
     int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
     int first;                // 1: store, 0: add into out
+    const int4 *ptab;         // merged launch: per-pass {c_begin, c_end, pass index, CTAs}; skew = table of all passes
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
     unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
 };
@@ -293,16 +294,27 @@ struct SbArgs {
 constexpr int SB_EP_PITCH = (SB_K / 2) % 2 == 1 ? SB_K + 4 : SB_K + 2;  // epilogue transpose: words per lane
 typedef unsigned long long sb_u64;  // one aligned register pair = two fp32 accumulators (FADD2 operand)
 
-template <typename OutT>
+template <typename OutT, bool MERGED>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // one pass per launch (ordered passes: deterministic fp32 sums), or all passes of the plan in one
+    // launch, pass = blockIdx.y (out zeroed beforehand, every pass adds with reductions: exact for u8 plans)
+    int c_begin = A.c_begin, c_end = A.c_end;
+    const int first = MERGED ? 0 : A.first;
+    const int32_t *skew = A.skew;
+    if constexpr (MERGED) {
+        const int4 pt = __ldg(A.ptab + blockIdx.y);      // {c_begin, c_end, pass index, CTAs of this pass}
+        if ((int)blockIdx.x >= pt.w) return;
+        c_begin = pt.x; c_end = pt.y;
+        skew = A.skew + (size_t)pt.z * A.ndm;
+    }
     const int blk = A.blk0 + blockIdx.x % A.nblk_run;
     const long long U0 = (long long)(blockIdx.x / A.nblk_run) * SB_T;
     const int d_first = blk * SB_ROWS;
     const int d_last = min(A.ndm, d_first + SB_ROWS) - 1;
     // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
-    if (U0 + SB_T <= (long long)__ldg(A.skew + d_first) || U0 >= (long long)__ldg(A.skew + d_last) + A.nsamp_out) return;
+    if (U0 + SB_T <= (long long)__ldg(skew + d_first) || U0 >= (long long)__ldg(skew + d_last) + A.nsamp_out) return;
 
     const float *in = A.in + (size_t)blockIdx.z * A.in_beam;
     const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
@@ -319,7 +331,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 #pragma unroll
         for (int k = 0; k < SB_K / 2; ++k) acc[j][k] = 0ull;
 
-    const int nchan = A.c_end - A.c_begin;
+    const int nchan = c_end - c_begin;
     const int nstages = (nchan + CB - 1) / CB;
 
     // Staging: warp w copies channel w of the stage (SB_CB == SB_WARPS); lane l copies logical chunks
@@ -332,8 +344,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     // that its L2 latency never sits in front of the copies
     auto load_meta = [&](int stage, int k) -> int2 {
         const int cc = warp + k * SB_WARPS;
-        const int c = A.c_begin + stage * CB + cc;
-        if (stage < nstages && cc < CB && c < A.c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
+        const int c = c_begin + stage * CB + cc;
+        if (stage < nstages && cc < CB && c < c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
         return make_int2(0, 0);
     };
     int2 mt[2] = {load_meta(0, 0), load_meta(0, 1)};
@@ -341,10 +353,10 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
         const int cc = warp + k * SB_WARPS;
-        const int c = A.c_begin + stage * CB + cc;
+        const int c = c_begin + stage * CB + cc;
         const int2 mt_cur = mt[k];
         mt[k] = load_meta(stage + 1, k);
-        if (stage < nstages && cc < CB && c < A.c_end) {
+        if (stage < nstages && cc < CB && c < c_end) {
             const int buf = stage % SB_STAGES;
             const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
             const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes + 16u * sb_phys(lane);
@@ -438,7 +450,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     for (int j = 0; j < SB_D; ++j) {
         const int d = d_first + warp * SB_D + j;
         if (d >= A.ndm) break;
-        const long long t0 = U0 - (long long)__ldg(A.skew + d);
+        const long long t0 = U0 - (long long)__ldg(skew + d);
         OutT *orow = out + (size_t)d * A.out_stride;
         const float *erow = ep + j * 32 * EP_PITCH;
         auto E = [&](int sidx) { return erow[(sidx / SB_K) * EP_PITCH + (sidx % SB_K)]; };
@@ -447,9 +459,9 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             if (t >= 0 && t < A.nsamp_out) {
                 if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
                     const int vi = __float2int_rn(E(sidx));
-                    orow[t] = A.first ? vi : orow[t] + vi;
+                    orow[t] = first ? vi : orow[t] + vi;
                 } else {
-                    if (A.first) orow[t] = E(sidx);
+                    if (first) orow[t] = E(sidx);
                     else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + t), "f"(E(sidx)) : "memory");
                 }
             }
@@ -465,7 +477,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                     const long long t = t0 + sidx;
                     if (t >= 0 && t + 3 < A.nsamp_out) {
                         const float x0 = E(sidx), x1 = E(sidx + 1), x2 = E(sidx + 2), x3 = E(sidx + 3);
-                        if (A.first) *reinterpret_cast<float4 *>(orow + t) = make_float4(x0, x1, x2, x3);
+                        if (first) *reinterpret_cast<float4 *>(orow + t) = make_float4(x0, x1, x2, x3);
                         else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
                                           ::"l"(orow + t), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
                     } else {
@@ -519,6 +531,7 @@ cudaError_t subband_upload(dedisp_plan *p) {
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_records, sb.records.data(), sb.records.size() * sizeof(uint64_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&sb.d_meta, sb.meta.size() * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_meta, sb.meta.data(), sb.meta.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&sb.d_ptab, std::max<size_t>(1, sb.passes.size()) * sizeof(int4));
     if (e == cudaSuccess) e = cudaMalloc(&sb.d_skew, sb.skew.size() * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_skew, sb.skew.data(), sb.skew.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     return e;
@@ -528,6 +541,8 @@ void subband_free(dedisp_plan *p) {
     if (p->sb.d_records) cudaFree(p->sb.d_records);
     if (p->sb.d_meta) cudaFree(p->sb.d_meta);
     if (p->sb.d_skew) cudaFree(p->sb.d_skew);
+    if (p->sb.d_ptab) cudaFree(p->sb.d_ptab);
+    p->sb.d_ptab = nullptr;
     if (p->d_conv) cudaFree(p->d_conv);
     p->sb.d_records = nullptr;
     p->sb.d_meta = nullptr;
@@ -540,9 +555,21 @@ static bool sb_needs_staging_copy(const dedisp_plan *p, const void *d_in, long l
     return p->dtype != DEDISP_F32 || ((uintptr_t)d_in & 15) != 0 || (in_stride & 3) != 0 || (b.n > 1 && (b.in_stride & 3) != 0);
 }
 
+// All passes in one launch? Measured (profiles/r1_paper_sweep.md): it pays only for plans cut into many
+// short passes (launch gaps and tile prologues dominate); long passes lose 2-5 % to idle CTAs and worse
+// L2 sharing. u8 plans (exact, order-independent sums) merge below 48 channels per pass on average;
+// fp plans only when the caller asked for it (dedisp_plan_set_pass_merge).
+static bool sb_merge_passes(const dedisp_plan *p) {
+    const size_t np = p->sb.passes.size();
+    if (np < 2) return false;
+    if (p->dtype == DEDISP_U8) return (size_t)p->nchans <= 48 * np;
+    return p->merge_fp_passes;
+}
+
 int subband_launches(const dedisp_plan *p, int resolved_kernel) {
     if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
-    return (int)p->sb.passes.size() + (p->dtype != DEDISP_F32 ? 1 : 0) + (p->dtype == DEDISP_U8 ? 1 : 0);
+    const bool merged = sb_merge_passes(p);   // + a memset, which is not a kernel
+    return (merged ? 1 : (int)p->sb.passes.size()) + (p->dtype != DEDISP_F32 ? 1 : 0) + (p->dtype == DEDISP_U8 ? 1 : 0);
 }
 
 cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams) {
@@ -611,10 +638,43 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (ring_bytes(cb) <= 227u * 1024u) { A.cb = cb; break; }
     size_t smem = ring_bytes(A.cb);
     smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * SB_EP_PITCH * sizeof(float));  // epilogue transpose region
-    auto kern = dedisp_subband_kernel<float>;   // u8 plans too: fp32 sums in place, converted after the last pass
+    auto kern = dedisp_subband_kernel<float, false>;   // u8 plans too: fp32 sums in place, converted after the last pass
+    auto kern_merged = dedisp_subband_kernel<float, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern_merged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const size_t pass_hi = p->sb_pass_hi < 0 ? sb.passes.size() : (size_t)p->sb_pass_hi;
+    A.ptab = nullptr;
+    const bool whole = p->sb_pass_lo == 0 && pass_hi == sb.passes.size() && A.blk0 == 0 && A.nblk_run == sb.nblk;
+    if (whole && sb.d_ptab && sb_merge_passes(p)) {
+        // all passes in ONE launch (blockIdx.y = pass): out is zeroed, every pass adds with L2 reductions.
+        // Exact integers in fp32 are order-independent, so u8 plans stay bit-reproducible; fp plans only
+        // take this path when asked to (dedisp_plan_set_pass_merge), their sums then vary in the last bits.
+        for (int bm = 0; bm < b.n; ++bm) {
+            e = cudaMemset2DAsync((char *)d_out + (size_t)bm * b.out_stride * 4, (size_t)out_stride * 4, 0, (size_t)nsamp_out * 4, (size_t)p->ndm, st);
+            if (e != cudaSuccess) return e;
+        }
+        long long maxcta = 0;
+        for (const SubbandPass &ps : sb.passes) maxcta = std::max(maxcta, ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * sb.nblk);
+        std::vector<int4> tab(sb.passes.size());
+        for (size_t g = 0; g < sb.passes.size(); ++g)
+            tab[g] = make_int4(sb.passes[g].c_begin, sb.passes[g].c_end, (int)g, (int)(((nsamp_out + sb.passes[g].max_skew + SB_T - 1) / SB_T) * sb.nblk));
+        // the table depends on nsamp_out: refresh the device copy when it changed (stream-ordered)
+        if (sb.ptab_nsamp != nsamp_out) {
+            e = cudaMemcpyAsync(sb.d_ptab, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return e;
+            e = cudaStreamSynchronize(st);   // tab is a local: the copy must finish before it goes away
+            if (e != cudaSuccess) return e;
+            p->sb.ptab_nsamp = nsamp_out;
+        }
+        A.ptab = sb.d_ptab;
+        A.skew = sb.d_skew;
+        A.c_begin = 0; A.c_end = 0; A.first = 0;
+        dim3 grid((unsigned)maxcta, (unsigned)sb.passes.size(), (unsigned)b.n);
+        kern_merged<<<grid, SB_THREADS, smem, st>>>(A);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    } else
     for (size_t i = (size_t)p->sb_pass_lo; i < pass_hi; ++i) {
         const size_t g = p->sb_reverse ? sb.passes.size() - 1 - i : i;   // any order: the first launched pass stores
         const SubbandPass &ps = sb.passes[g];

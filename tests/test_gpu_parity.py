@@ -199,3 +199,20 @@ def test_execute_host_matches_oracle(name):
         assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"{name}/execute_host seed {seed}")
     if name == "c3s":
         assert plan.num_subbands() > 1 and (cfg.nsamp_out + plan.max_shift) % 4 == 0
+
+
+@pytest.mark.parametrize("name", ["c3s", "c4s", "paper"])
+def test_merged_passes_match_oracle(name):
+    """dedisp_plan_set_pass_merge: all SUBBAND passes in one launch, partial sums added with L2
+    reductions in any order. fp plans stay within the tolerance; u8 plans ("paper" merges on its own:
+    many short passes) stay bit-exact because their fp32 partial sums are exact integers."""
+    cfg = SMALL[name]
+    plan = _plan_with(cfg, P.KERNEL_SUBBAND)
+    plan.set_pass_merge(True)
+    assert plan.num_subbands() > 1
+    x, tab, _ = make_case(cfg)
+    ref = oracle_rows(cfg, x.cpu().numpy())
+    for _ in range(2):                       # twice: the merged path zeroes out itself
+        out = plan.execute(x, cfg.nsamp_out)
+        torch.cuda.synchronize()
+        assert_matches_oracle(cfg, out, ref, what=f"{name}/merged")
