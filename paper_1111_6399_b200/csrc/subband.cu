@@ -223,7 +223,8 @@ static_assert(SB_STAGES >= 4, "ring depth: prefetch distance SB_STAGES - 3 >= 1"
 #ifndef SB_CB_MAX_CFG
 #define SB_CB_MAX_CFG SB_WARPS
 #endif
-constexpr int SB_CB_MAX = SB_CB_MAX_CFG;   // channels per stage are chosen at launch (as many as fit): warp w stages w, w + SB_WARPS
+constexpr int SB_CB_MAX = SB_CB_MAX_CFG;
+static_assert(SB_CB_MAX <= SB_WARPS, "staging: at most one channel per warp and stage");   // channels per stage are chosen at launch (as many as fit)
 static_assert(SB_CB <= SB_WARPS, "the smallest stage: one channel per staging warp");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
@@ -342,20 +343,19 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
     // meta (window base, chunk count) of the channel this warp stages next: loaded one stage ahead so
     // that its L2 latency never sits in front of the copies
-    auto load_meta = [&](int stage, int k) -> int2 {
-        const int cc = warp + k * SB_WARPS;
+    auto load_meta = [&](int stage) -> int2 {
+        const int cc = warp;
         const int c = c_begin + stage * CB + cc;
         if (stage < nstages && cc < CB && c < c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
         return make_int2(0, 0);
     };
-    int2 mt[2] = {load_meta(0, 0), load_meta(0, 1)};
+    int2 mt = load_meta(0);
     auto issue = [&](int stage, unsigned full_bar) {
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-        const int cc = warp + k * SB_WARPS;
+        {
+        const int cc = warp;                              // at most one channel per warp and stage (CB <= SB_WARPS)
         const int c = c_begin + stage * CB + cc;
-        const int2 mt_cur = mt[k];
-        mt[k] = load_meta(stage + 1, k);
+        const int2 mt_cur = mt;
+        mt = load_meta(stage + 1);
         if (stage < nstages && cc < CB && c < c_end) {
             const int buf = stage % SB_STAGES;
             const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
