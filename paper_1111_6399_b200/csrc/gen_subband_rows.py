@@ -197,7 +197,7 @@ def generate_joint(D, K, S, G=None):
     instruction cache (measured on c3: 16-18 of 122 for D = G = 3, S = 4), so the tables may be large."""
     import itertools
     G = D if G is None else G
-    assert D % G == 0 and (S + 2) ** G <= 256
+    assert D % G == 0 and ((S + 2) ** G <= 256 or G == D)   # 8 bits per group; a single group owns the whole word
     K2, OM = K // 2, S + 1
     NP = (K + OM + 1) // 2
     NG = D // G
@@ -218,7 +218,7 @@ def generate_joint(D, K, S, G=None):
     for m in range(NP):
         L.append("ld.shared.b64 w%d, [%s+%d];" % (m, SA, 8 * m))
     for g in range(NG):
-        L.append("bfe.u32 t%d, %s, %d, 8;" % (g, PID, 8 * g))
+        L.append("bfe.u32 t%d, %s, %d, %d;" % (g, PID, 8 * g, 8 if NG > 1 else 16))
     for m in range(NP):
         L.append("mov.b64 {lf%d, hf%d}, w%d;" % (m, m, m))
     L.append("brx.idx.uni t0, TP0;")

@@ -77,9 +77,10 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
                         const int o = (sc[d] - sref[d]) - rbase - AUNIT * a;
                         if (SB_JOINT) {   // 8 bits per dispatch group: pattern id, the group's first row most significant
+                            constexpr uint32_t FM = SB_G == SB_D ? 0xffffu : 255u;   // field: 8 bits per group, 16 for a single group
                             const int g = j / SB_G, sh = 8 * g;
-                            const uint32_t id = ((lo >> sh) & 255u) * (SB_S + 2) + (uint32_t)o;
-                            lo = (lo & ~(255u << sh)) | (id << sh);
+                            const uint32_t id = ((lo >> sh) & FM) * (SB_S + 2) + (uint32_t)o;
+                            lo = (lo & ~(FM << sh)) | (id << sh);
                         } else {
                             lo |= (uint32_t)o << (4 * j);
                         }
@@ -193,7 +194,7 @@ long long subband_verify_records(const dedisp_plan *p) {
                 const int a = (int)((rec >> 32) & 0xffff);
                 int o;
                 if (SB_JOINT) {
-                    uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
+                    uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & (SB_G == SB_D ? 0xffffu : 255u);
                     for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
                     o = (int)(id % (SB_S + 2));
                 } else {
