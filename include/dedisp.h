@@ -134,8 +134,10 @@ int dedisp_plan_set_kernel(dedisp_plan *plan, int kernel);
 int dedisp_plan_set_pass_merge(dedisp_plan *plan, int on);
 /* The kernel dedisp_execute will launch for this plan (resolved, never AUTO). */
 int dedisp_plan_get_kernel(const dedisp_plan *plan);
-/* Sub-band layout of the SUBBAND kernel: number of passes G (0 if the plan has none) and, if
- * h_first_chan != NULL, the G+1 channel boundaries. */
+/* Sub-band layout of the SUBBAND kernel: number of sub-bands G (0 if the plan has none) and, if
+ * h_first_chan != NULL, the G+1 channel boundaries. A plan whose DM step changes (e.g. 0.1 / 0.25 /
+ * 0.5) cuts its DM rows into ranges with one partition each; these two calls describe the first
+ * range, dedisp_plan_launches_per_execute counts the launches of all of them. */
 int dedisp_plan_num_subbands(const dedisp_plan *plan);
 int dedisp_plan_get_subbands(const dedisp_plan *plan, int *h_first_chan /* [G+1] */);
 /* Host check used by the CPU tests: rebuild s(c,d) for every (c,d) from the SUBBAND kernel's packed

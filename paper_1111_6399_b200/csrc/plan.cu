@@ -151,7 +151,7 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
     // sub-bands in pass order on a second stream and let pass g start as soon as its rows have landed,
     // so that most of the H2D transfer hides under the earlier passes.
     const bool overlap = resolve_kernel(p) == DEDISP_KERNEL_SUBBAND && p->dtype == DEDISP_F32 && (nsamp_in & 3) == 0 &&
-                         p->sb.passes.size() > 1;
+                         p->sb.passes.size() > 1 && p->sb.nranges == 1;
     if (overlap) {
         if (!p->host_copy_st) {
             e = cudaStreamCreateWithFlags(&p->host_copy_st, cudaStreamNonBlocking);
@@ -277,14 +277,19 @@ int dedisp_plan_get_kernel(const dedisp_plan *p) { return p ? resolve_kernel(p) 
 
 int dedisp_plan_num_subbands(const dedisp_plan *p) {
     if (!p) return -1;
-    return p->sb.ok ? (int)p->sb.passes.size() : 0;
+    if (!p->sb.ok) return 0;
+    int n = 0;   // sub-bands of the first DM range (plans with a changing DM step have one partition per range)
+    for (const SubbandPass &ps : p->sb.passes) n += ps.blk_begin == 0;
+    return n;
 }
 
 int dedisp_plan_get_subbands(const dedisp_plan *p, int *h_first_chan) {
     if (!p || !h_first_chan) return DEDISP_EINVAL;
     if (!p->sb.ok) return DEDISP_EUNSUPPORTED;
-    for (size_t g = 0; g < p->sb.passes.size(); ++g) h_first_chan[g] = p->sb.passes[g].c_begin;
-    h_first_chan[p->sb.passes.size()] = p->nchans;
+    int n = 0;
+    for (const SubbandPass &ps : p->sb.passes)
+        if (ps.blk_begin == 0) h_first_chan[n++] = ps.c_begin;
+    h_first_chan[n] = p->nchans;
     return DEDISP_OK;
 }
 

@@ -73,13 +73,16 @@ constexpr int SB_NCH_MAX = SB_JOINT ? ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 
 
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;
-    int max_skew = 0;                 // max_d s(c_ref, d)
+    int max_skew = 0;                 // max over the pass's DM rows of s(c_ref, d)
+    int blk_begin = 0, blk_end = 0;   // DM blocks this pass covers (a plan may cut its DM blocks into ranges)
+    bool first = false;               // first pass of its DM range: stores instead of adding
 };
 
 struct SubbandGeom {
     bool ok = false;
     std::vector<SubbandPass> passes;
     int ngroups = 0, nblk = 0;
+    int nranges = 0;                  // DM-block ranges, each with its own sub-band partition (1 for uniform DM plans)
     // per (channel, group): low word = SB_D 4-bit offsets o_j (per-row mode) or the joint pattern id
     // (o_0*(S+2) + o_1)*(S+2) + ..., high word = window base a in 16-byte chunks / 8-byte pairs (subband.cu)
     std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]

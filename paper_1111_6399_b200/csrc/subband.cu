@@ -36,14 +36,14 @@ inline int floor4(int v) { return v & ~3; }  // toward -inf, two's complement
 // Residual-delay geometry of channels [cb, ce) against reference channel cr. Returns false if some
 // group's in-window offsets would exceed SB_OMAX or a block's staged window exceeds SB_NCH_MAX.
 // With `emit`, writes records/meta for those channels.
-bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
+bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, int b1) {
     const int ndm = p->ndm, ngroups = p->sb.ngroups, nblk = p->sb.nblk;
     const int32_t *sref = p->shifts.data() + (size_t)cr * ndm;
     const int gslots = nblk * SB_WARPS;
     std::vector<int> gmin(gslots), gmax(gslots);
     for (int c = cb; c < ce; ++c) {
         const int32_t *sc = p->shifts.data() + (size_t)c * ndm;
-        for (int q = 0; q < ngroups; ++q) {
+        for (int q = b0 * SB_WARPS; q < std::min(ngroups, b1 * SB_WARPS); ++q) {
             int mn = INT32_MAX, mx = INT32_MIN;
             for (int j = 0; j < SB_D; ++j) {
                 const int d = std::min(q * SB_D + j, ndm - 1);
@@ -54,8 +54,8 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit) {
             gmin[q] = mn;
             gmax[q] = mx;
         }
-        for (int q = ngroups; q < gslots; ++q) { gmin[q] = gmin[ngroups - 1]; gmax[q] = gmax[ngroups - 1]; }
-        for (int b = 0; b < nblk; ++b) {
+        for (int q = std::max(ngroups, b0 * SB_WARPS); q < std::min(gslots, b1 * SB_WARPS); ++q) { gmin[q] = gmin[ngroups - 1]; gmax[q] = gmax[ngroups - 1]; }
+        for (int b = b0; b < b1; ++b) {
             int bmin = INT32_MAX;
             for (int w = 0; w < SB_WARPS; ++w) bmin = std::min(bmin, gmin[b * SB_WARPS + w]);
             const int rbase = floor4(bmin);
@@ -132,42 +132,68 @@ void subband_build(dedisp_plan *p) {
     const size_t gslots = (size_t)sb.nblk * SB_WARPS;
     if ((double)nchans * gslots * 8.0 > 4.0e9) return;  // record table would not fit sensibly
     if (p->dtype == DEDISP_U8 && (double)nchans * 255.0 >= 16777216.0) return;  // fp32 sums must stay exact
-    // greedy: extend each sub-band as far as the geometry admits (exponential then binary search)
-    int cb = 0;
-    while (cb < nchans) {
-        auto ok = [&](int ce) { return pass_geometry(p, cb, ce, pick_ref(p, cb, ce), false); };
-        if (!ok(cb + 1)) return;  // a single channel against itself always has r = 0; defensive
-        int good = cb + 1, step = 1;
-        while (good < nchans) {
-            const int trial = std::min(nchans, good + step);
-            if (ok(trial)) { good = trial; step *= 2; } else break;
+    // DM-block ranges: a plan whose DM step changes (c4: 0.1 / 0.25 / 0.5) would force the sub-band width
+    // of its coarsest part on all rows; blocks are therefore grouped by their adjacent-row delay step at
+    // the lowest channel (within a factor 1.5) and every range gets its own sub-band partition.
+    std::vector<int> range_begin;
+    {
+        const int32_t *slast = p->shifts.data() + (size_t)(nchans - 1) * ndm;
+        double lo = 0, hi = 0;
+        for (int b = 0; b < sb.nblk; ++b) {
+            const int d0 = b * SB_ROWS, d1 = std::min(ndm, d0 + SB_ROWS);
+            double step = d1 - d0 > 1 ? (double)(slast[d1 - 1] - slast[d0]) / (d1 - d0 - 1) : 0.0;
+            step = std::max(step, 1.0);
+            if (b == 0 || std::max(hi, step) > 1.5 * std::min(lo, step)) { range_begin.push_back(b); lo = hi = step; }
+            else { lo = std::min(lo, step); hi = std::max(hi, step); }
         }
-        int bad = std::min(nchans, good + step);  // first known-bad (or nchans if all good)
-        if (good < nchans) {
-            int lo = good, hi = bad;  // ok(lo) true, ok(hi) false
-            while (hi - lo > 1) {
-                const int m = (lo + hi) / 2;
-                if (ok(m)) lo = m; else hi = m;
+        if (range_begin.size() > 8) range_begin.assign(1, 0);   // erratic DM list: one range
+        range_begin.push_back(sb.nblk);
+    }
+    sb.nranges = (int)range_begin.size() - 1;
+    for (int r = 0; r < sb.nranges; ++r) {
+        const int b0 = range_begin[r], b1 = range_begin[r + 1];
+        // greedy: extend each sub-band as far as the geometry admits (exponential then binary search)
+        int cb = 0;
+        bool first = true;
+        while (cb < nchans) {
+            auto ok = [&](int ce) { return pass_geometry(p, cb, ce, pick_ref(p, cb, ce), false, b0, b1); };
+            if (!ok(cb + 1)) { sb = SubbandGeom(); return; }  // a single channel against itself always has r = 0; defensive
+            int good = cb + 1, step = 1;
+            while (good < nchans) {
+                const int trial = std::min(nchans, good + step);
+                if (ok(trial)) { good = trial; step *= 2; } else break;
             }
-            good = lo;
+            int bad = std::min(nchans, good + step);  // first known-bad (or nchans if all good)
+            if (good < nchans) {
+                int lo = good, hi = bad;  // ok(lo) true, ok(hi) false
+                while (hi - lo > 1) {
+                    const int m = (lo + hi) / 2;
+                    if (ok(m)) lo = m; else hi = m;
+                }
+                good = lo;
+            }
+            SubbandPass ps;
+            ps.c_begin = cb;
+            ps.c_end = good;
+            ps.c_ref = pick_ref(p, cb, good);
+            ps.blk_begin = b0;
+            ps.blk_end = b1;
+            ps.first = first;
+            first = false;
+            sb.passes.push_back(ps);
+            cb = good;
+            if (sb.passes.size() > 2048) { sb = SubbandGeom(); return; }  // hopelessly coarse plan: use TILED
         }
-        SubbandPass ps;
-        ps.c_begin = cb;
-        ps.c_end = good;
-        ps.c_ref = pick_ref(p, cb, good);
-        sb.passes.push_back(ps);
-        cb = good;
-        if (sb.passes.size() > 512) { sb.passes.clear(); return; }  // hopelessly coarse plan: use TILED
     }
     sb.records.assign((size_t)nchans * gslots, 0);
     sb.meta.assign((size_t)nchans * sb.nblk * 2, 0);
     sb.skew.assign(sb.passes.size() * (size_t)ndm, 0);
     for (size_t g = 0; g < sb.passes.size(); ++g) {
         SubbandPass &ps = sb.passes[g];
-        if (!pass_geometry(p, ps.c_begin, ps.c_end, ps.c_ref, true)) { sb = SubbandGeom(); return; }
+        if (!pass_geometry(p, ps.c_begin, ps.c_end, ps.c_ref, true, ps.blk_begin, ps.blk_end)) { sb = SubbandGeom(); return; }
         const int32_t *sref = p->shifts.data() + (size_t)ps.c_ref * ndm;
         std::memcpy(sb.skew.data() + g * (size_t)ndm, sref, (size_t)ndm * sizeof(int32_t));
-        ps.max_skew = sref[ndm - 1];
+        ps.max_skew = sref[std::min(ndm, ps.blk_end * SB_ROWS) - 1];
     }
     // the kernel's dynamic shared memory (ring + records) must fit the 227 KB a CTA may opt into
     if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + sb.max_nch / SB_P + 1) * 16 + SB_WARPS * 8 + 16) > 227u * 1024u) { sb = SubbandGeom(); return; }
@@ -183,12 +209,12 @@ long long subband_verify_records(const dedisp_plan *p) {
     const int ndm = p->ndm;
     const size_t gslots = (size_t)sb.nblk * SB_WARPS;
     long long bad = 0;
-    std::vector<char> seen(p->nchans, 0);
+    std::vector<int> seen(p->nchans, 0);   // DM blocks that cover channel c: every channel exactly once per block
     for (size_t g = 0; g < sb.passes.size(); ++g) {
         const SubbandPass &ps = sb.passes[g];
         for (int c = ps.c_begin; c < ps.c_end; ++c) {
-            seen[c]++;
-            for (int d = 0; d < ndm; ++d) {
+            seen[c] += ps.blk_end - ps.blk_begin;
+            for (int d = ps.blk_begin * SB_ROWS; d < std::min(ndm, ps.blk_end * SB_ROWS); ++d) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
                 const uint64_t rec = sb.records[(size_t)c * gslots + q];
                 const int a = (int)((rec >> 32) & 0xffff);
@@ -208,7 +234,7 @@ long long subband_verify_records(const dedisp_plan *p) {
             }
         }
     }
-    for (int c = 0; c < p->nchans; ++c) bad += seen[c] != 1;
+    for (int c = 0; c < p->nchans; ++c) bad += seen[c] != sb.nblk;
     return bad;
 }
 
@@ -628,8 +654,9 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.ndm = p->ndm;
     A.nblk = sb.nblk;
     A.gslots = sb.nblk * SB_WARPS;
-    A.blk0 = p->sb_blk_begin;
-    A.nblk_run = (p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end) - p->sb_blk_begin;
+    const int run_b0 = p->sb_blk_begin, run_b1 = p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end;   // caller's DM-block range
+    A.blk0 = run_b0;
+    A.nblk_run = run_b1 - run_b0;
     A.slot_chunks = sb_phys(sb.max_nch) + 1;
     A.zero = 0;
     // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
@@ -646,8 +673,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     if (e != cudaSuccess) return e;
     const size_t pass_hi = p->sb_pass_hi < 0 ? sb.passes.size() : (size_t)p->sb_pass_hi;
     A.ptab = nullptr;
-    const bool whole = p->sb_pass_lo == 0 && pass_hi == sb.passes.size() && A.blk0 == 0 && A.nblk_run == sb.nblk;
-    if (whole && sb.d_ptab && sb_merge_passes(p)) {
+    const bool whole = p->sb_pass_lo == 0 && pass_hi == sb.passes.size() && run_b0 == 0 && run_b1 == sb.nblk;
+    if (whole && sb.nranges == 1 && sb.d_ptab && sb_merge_passes(p)) {
         // all passes in ONE launch (blockIdx.y = pass): out is zeroed, every pass adds with L2 reductions.
         // Exact integers in fp32 are order-independent, so u8 plans stay bit-reproducible; fp plans only
         // take this path when asked to (dedisp_plan_set_pass_merge), their sums then vary in the last bits.
@@ -682,7 +709,10 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         A.skew = sb.d_skew + g * (size_t)p->ndm;
         A.c_begin = ps.c_begin;
         A.c_end = ps.c_end;
-        A.first = i == 0;
+        A.blk0 = std::max(run_b0, ps.blk_begin);                     // the pass's DM range, clipped to the caller's
+        A.nblk_run = std::min(run_b1, ps.blk_end) - A.blk0;
+        if (A.nblk_run <= 0) continue;
+        A.first = sb.nranges == 1 ? i == 0 : ps.first;               // one range: any order, the first launched stores
         const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
         dim3 grid((unsigned)(ntiles * A.nblk_run), 1, (unsigned)b.n);
         if (p->pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
@@ -694,7 +724,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (e != cudaSuccess) return e;
     }
     if (p->dtype == DEDISP_U8 && pass_hi == sb.passes.size()) {   // last pass done for these rows
-        const int d0 = std::min(p->ndm, A.blk0 * SB_ROWS), d1 = std::min(p->ndm, (A.blk0 + A.nblk_run) * SB_ROWS);
+        const int d0 = std::min(p->ndm, run_b0 * SB_ROWS), d1 = std::min(p->ndm, run_b1 * SB_ROWS);
         for (int r0 = d0; r0 < d1; r0 += 32768) {   // grid.y <= 65535
             dim3 grid((unsigned)((nsamp_out + 255) / 256), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
             dedisp_f32_to_i32_inplace_kernel<<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
