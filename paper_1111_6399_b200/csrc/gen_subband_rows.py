@@ -251,7 +251,7 @@ def generate_joint(D, K, S, G=None):
 
 if __name__ == "__main__" and (len(sys.argv) < 2 or sys.argv[1] == "joint"):
     a = [int(x) for x in sys.argv[2:]]
-    D, K, S = a[:3] if len(a) >= 3 else (4, 26, 4)
+    D, K, S = a[:3] if len(a) >= 3 else (4, 26, 5)
     G = a[3] if len(a) > 3 else (2 if len(a) < 3 else D)
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows.inc")
     with open(path, "w") as f:

@@ -40,7 +40,7 @@ struct TiledGeom {
 #define SB_OMAX_CFG 12
 #endif
 #ifndef SB_S_CFG
-#define SB_S_CFG 4
+#define SB_S_CFG 5
 #endif
 #ifndef SB_WARPS_CFG
 #define SB_WARPS_CFG 12
