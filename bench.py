@@ -154,7 +154,7 @@ def run_reference(args, cfg):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per dedisp_execute from the committed ncu --set full
 # capture (profiles/), keyed by (workload, resolved kernel); None until captured.
-NCU_TRAFFIC_BYTES = {("c3_meerkat_f32", "subband"): 64.4e9}   # profiles/r1_subband.md: 33.1 GB read + 31.3 GB written per execute (15 passes)
+NCU_TRAFFIC_BYTES = {("c3_meerkat_f32", "subband"): 51.8e9}   # profiles/r1_subband.md: 26.7 GB read + 25.1 GB written per execute (12 passes)
 
 
 def run_ours(args, cfg):
