@@ -19,25 +19,13 @@ struct TiledGeom {
 // SUBBAND kernel (subband.cu): exact sub-band re-skewed multi-pass with register-window reuse.
 // Thread tile = SB_D DM rows x SB_K consecutive samples; warp = one DM group (SB_D rows) x 32 lanes;
 // CTA = SB_WARPS groups x SB_T samples in the pass's skewed time coordinate u = t + s(c_ref, d).
-// Two generated channel bodies exist (gen_subband_rows.py): SB_JOINT = 1 dispatches ONCE per channel on
-// the joint offset pattern of the thread's rows (window in 8-byte pairs, offsets 0..SB_S+1); SB_JOINT = 0
-// dispatches per row (window in 16-byte chunks, offsets 0..SB_OMAX).
-#ifndef SB_JOINT_CFG
-#define SB_JOINT_CFG 1
-#endif
+// The channel loop is generated threaded code (gen_subband_rows.py -> subband_rows.inc): per channel
+// one jump per group of SB_G rows on the group's joint offset pattern (window in 8-byte pairs, in-window
+// offsets 0..SB_S+1).
 #ifndef SB_D_CFG
-#if SB_JOINT_CFG
 #define SB_D_CFG 4
 #define SB_G_CFG 2
-#else
-#define SB_D_CFG 3
-#endif
-#if SB_JOINT_CFG
 #define SB_K_CFG 26
-#else
-#define SB_K_CFG 28
-#endif
-#define SB_OMAX_CFG 12
 #endif
 #ifndef SB_S_CFG
 #define SB_S_CFG 5
@@ -45,31 +33,26 @@ struct TiledGeom {
 #ifndef SB_WARPS_CFG
 #define SB_WARPS_CFG 12
 #endif
-constexpr bool SB_JOINT = SB_JOINT_CFG != 0;
 constexpr int SB_D = SB_D_CFG;
 constexpr int SB_K = SB_K_CFG;
 constexpr int SB_T = 32 * SB_K;       // u-samples per CTA tile
 constexpr int SB_WARPS = SB_WARPS_CFG; // DM groups per CTA (one warp each)
 constexpr int SB_ROWS = SB_D * SB_WARPS;
-#ifndef SB_G_CFG
-#define SB_G_CFG SB_D_CFG
-#endif
-constexpr int SB_G = SB_G_CFG;        // joint: rows per dispatch group (SB_D: one jump per channel)
-constexpr int SB_S = SB_S_CFG;        // joint: largest spread of the residual delay over a thread's rows
-constexpr int SB_OMAX = SB_JOINT ? SB_S + 1 : SB_OMAX_CFG;  // largest in-window offset a row may have
-constexpr int SB_P = SB_K / 4;        // per-row mode: 16-byte chunks per lane (pad period if even)
-constexpr int SB_WCHUNKS = (SB_K + SB_OMAX + 3) / 4;   // per-row mode: 16-byte chunks a thread loads per channel
-constexpr int SB_WPAIRS = (SB_K + SB_OMAX + 1) / 2;    // joint mode: 8-byte pairs a thread loads per channel
+constexpr int SB_G = SB_G_CFG;        // rows per dispatch group
+constexpr int SB_S = SB_S_CFG;        // largest spread of the residual delay over a thread's rows
+constexpr int SB_OMAX = SB_S + 1;     // largest in-window offset a row may have
+constexpr int SB_WPAIRS = (SB_K + SB_OMAX + 1) / 2;    // 8-byte pairs a thread loads per channel
+constexpr int SB_REC_STRIDE = SB_WARPS * 8;            // bytes between a warp's records of consecutive staged channels
 #ifndef SB_CB_CFG
 #define SB_CB_CFG 8
 #endif
-constexpr int SB_CB = SB_CB_CFG;      // channels per pipeline stage (one staging warp each)
+constexpr int SB_CB = SB_CB_CFG;      // smallest number of channels per pipeline stage (one staging warp each)
 #ifndef SB_STAGES_CFG
 #define SB_STAGES_CFG 4
 #endif
 constexpr int SB_STAGES = SB_STAGES_CFG;
-// staged 16-byte chunks per channel the slot can hold (logical), a multiple of 32
-constexpr int SB_NCH_MAX = SB_JOINT ? ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 * 32 : SB_P * 32 + 96;
+// staged 16-byte chunks per channel the slot can hold, a multiple of 32
+constexpr int SB_NCH_MAX = ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 * 32;
 
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;
@@ -83,8 +66,8 @@ struct SubbandGeom {
     std::vector<SubbandPass> passes;
     int ngroups = 0, nblk = 0;
     int nranges = 0;                  // DM-block ranges, each with its own sub-band partition (1 for uniform DM plans)
-    // per (channel, group): low word = SB_D 4-bit offsets o_j (per-row mode) or the joint pattern id
-    // (o_0*(S+2) + o_1)*(S+2) + ..., high word = window base a in 16-byte chunks / 8-byte pairs (subband.cu)
+    // per (channel, group): low word = joint pattern ids, 8 bits per dispatch group (group 0 lowest):
+    // (o_a*(S+2) + o_b)..., high word = window base a in 8-byte pairs (subband.cu)
     std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]
     // per (channel, block): {window base r (multiple of 4, relative to u), chunks to stage}
     std::vector<int32_t> meta;        // [nchans][nblk][2]

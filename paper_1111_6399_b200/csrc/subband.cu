@@ -18,11 +18,12 @@
 // Per channel a thread: its record (prefetched one channel ahead), SB_WPAIRS LDS.64 of the window,
 // then per group of SB_G rows ONE warp-uniform indirect branch on the group's joint offset pattern
 // into a body with static register operands (registers cannot be indexed dynamically): SB_K/2 FADD2
-// per row with an even offset, SB_K scalar FADD per row with an odd one. That body is generated
-// inline PTX: see gen_subband_rows.py for why and subband_rows.inc for the text (SB_JOINT_CFG=0
-// selects the older per-row dispatch). Around it: an SB_STAGES-deep ring filled by TMA bulk copies
-// and handed over with mbarrier full/empty pairs (no CTA barrier in the loop), and a transposing
-// epilogue that writes out with vector stores / red.global.add.v4.f32.
+// per row with an even offset, SB_K scalar FADD per row with an odd one. The channel loop of a whole
+// pipeline stage is one generated inline-PTX statement of threaded code: the last group's bodies
+// prefetch the next channel's window under their adds and jump straight into its first group (see
+// gen_subband_rows.py for why and subband_rows.inc for the text). Around it: an SB_STAGES-deep ring
+// filled by TMA bulk copies and handed over with mbarrier full/empty pairs (no CTA barrier in the
+// loop), and a transposing epilogue that writes out with vector stores / red.global.add.v4.f32.
 #include <algorithm>
 #include <cstring>
 #include <type_traits>
@@ -59,15 +60,15 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
             int bmin = INT32_MAX;
             for (int w = 0; w < SB_WARPS; ++w) bmin = std::min(bmin, gmin[b * SB_WARPS + w]);
             const int rbase = floor4(bmin);
-            // window base of a group inside the block's staged region: 16-byte chunks (per-row mode) or
-            // 8-byte pairs (joint mode); what is left of the residual delays are the in-window offsets
-            constexpr int AUNIT = SB_JOINT ? 2 : 4;
+            // window base of a group inside the block's staged region in 8-byte pairs; what is left of
+            // the residual delays are the in-window offsets
+            constexpr int AUNIT = 2;
             int amax = 0;
             for (int w = 0; w < SB_WARPS; ++w) {
                 const int q = b * SB_WARPS + w;
                 const int a = (gmin[q] - rbase) / AUNIT;
                 if (gmax[q] - rbase - AUNIT * a > SB_OMAX) return false;
-                if (SB_JOINT && gmax[q] - gmin[q] > SB_S) return false;
+                if (gmax[q] - gmin[q] > SB_S) return false;
                 amax = std::max(amax, a);
                 if (emit) {
                     uint64_t rec = (uint64_t)a << 32;
@@ -76,20 +77,16 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
                     for (int j = 0; j < SB_D; ++j) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
                         const int o = (sc[d] - sref[d]) - rbase - AUNIT * a;
-                        if (SB_JOINT) {   // 8 bits per dispatch group: pattern id, the group's first row most significant
-                            constexpr uint32_t FM = SB_G == SB_D ? 0xffffu : 255u;   // field: 8 bits per group, 16 for a single group
-                            const int g = j / SB_G, sh = 8 * g;
-                            const uint32_t id = ((lo >> sh) & FM) * (SB_S + 2) + (uint32_t)o;
-                            lo = (lo & ~(FM << sh)) | (id << sh);
-                        } else {
-                            lo |= (uint32_t)o << (4 * j);
-                        }
+                        // 8 bits per dispatch group: pattern id, the group's first row most significant
+                        const int g = j / SB_G, sh = 8 * g;
+                        const uint32_t id = ((lo >> sh) & 255u) * (SB_S + 2) + (uint32_t)o;
+                        lo = (lo & ~(255u << sh)) | (id << sh);
                     }
                     p->sb.records[(size_t)c * gslots + q] = rec | lo;
                 }
             }
             // staged 16-byte chunks: the furthest lane of the furthest group must find its whole window
-            const int nch = SB_JOINT ? (2 * amax + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 : amax + SB_P * 31 + SB_WCHUNKS;
+            const int nch = (2 * amax + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
             if (nch > SB_NCH_MAX || amax > 0xffff) return false;
             if (emit) {
                 p->sb.meta[((size_t)c * nblk + b) * 2 + 0] = rbase;
@@ -196,7 +193,7 @@ void subband_build(dedisp_plan *p) {
         ps.max_skew = sref[std::min(ndm, ps.blk_end * SB_ROWS) - 1];
     }
     // the kernel's dynamic shared memory (ring + records) must fit the 227 KB a CTA may opt into
-    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + sb.max_nch / SB_P + 1) * 16 + SB_WARPS * 8 + 16) > 227u * 1024u) { sb = SubbandGeom(); return; }
+    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + 1) * 16 + SB_REC_STRIDE + 16) + SB_REC_STRIDE > 227u * 1024u) { sb = SubbandGeom(); return; }
     sb.ok = true;
 }
 
@@ -218,18 +215,13 @@ long long subband_verify_records(const dedisp_plan *p) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
                 const uint64_t rec = sb.records[(size_t)c * gslots + q];
                 const int a = (int)((rec >> 32) & 0xffff);
-                int o;
-                if (SB_JOINT) {
-                    uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & (SB_G == SB_D ? 0xffffu : 255u);
-                    for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
-                    o = (int)(id % (SB_S + 2));
-                } else {
-                    o = (int)((rec >> (4 * j)) & 15);
-                }
+                uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
+                for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
+                const int o = (int)(id % (SB_S + 2));
                 const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
                 const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
-                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + (SB_JOINT ? 2 : 4) * a + o;
-                const int need = SB_JOINT ? (2 * a + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 : a + SB_P * 31 + SB_WCHUNKS;
+                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 2 * a + o;
+                const int need = (2 * a + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
                 if (s != p->shifts[(size_t)c * ndm + d] || need > nch || (rbase & 3) || o > SB_OMAX) ++bad;
             }
         }
@@ -255,13 +247,9 @@ static_assert(SB_CB_MAX <= SB_WARPS, "staging: at most one channel per warp and 
 static_assert(SB_CB <= SB_WARPS, "the smallest stage: one channel per staging warp");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
-// Staged layout: lanes are SB_P chunks apart. Odd SB_P: the plain layout is already conflict-free for
-// LDS.128 (8 consecutive lanes hit 8 different 16-byte bank groups) and a channel's window is ONE
-// contiguous TMA bulk copy. Even SB_P: one pad chunk per SB_P chunks, copied with 16-byte cp.async.
-constexpr bool SB_PADDED = !SB_JOINT && (SB_P % 2) == 0;
-__host__ __device__ constexpr int sb_phys(int chunk) { return SB_PADDED ? chunk + chunk / SB_P : chunk; }
-static_assert(SB_JOINT || ((!SB_PADDED || (SB_P & (SB_P - 1)) == 0) && SB_P >= 2 && SB_K % 4 == 0 && SB_D * 4 <= 32), "tile constants");
-static_assert(!SB_JOINT || (SB_K % 2 == 0 && (SB_K / 2) % 2 == 1), "joint mode: K/2 odd (LDS.64 conflict-free in the plain layout)");
+// Staged layout: a channel's window is plain and contiguous (ONE TMA bulk copy); lanes are SB_K words
+// apart and SB_K/2 is odd, so LDS.64 is conflict-free (16 consecutive lanes hit 16 different bank pairs).
+static_assert(SB_K % 2 == 0 && (SB_K / 2) % 2 == 1, "K/2 odd: LDS.64 conflict-free in the plain layout");
 static_assert(SB_WARPS % 2 == 0 && SB_NCH_MAX % 32 == 0, "tile constants");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
@@ -316,7 +304,6 @@ struct SbArgs {
     int first;                // 1: store, 0: add into out
     const int4 *ptab;         // merged launch: per-pass {c_begin, c_end, pass index, CTAs}; skew = table of all passes
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
-    unsigned zero;            // always 0, opaque to the compiler (used by gen_subband_rows.py odd_mode 1 only)
 };
 
 constexpr int SB_EP_PITCH = (SB_K / 2) % 2 == 1 ? SB_K + 4 : SB_K + 2;  // epilogue transpose: words per lane
@@ -349,9 +336,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const int CB = A.cb;
     const unsigned stage_bytes = CB * slot_bytes;
     unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
-    uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS]
-    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + (SB_JOINT ? 4u * SB_K * lane : 16u * sb_phys(SB_P * lane));
-    const unsigned zero = A.zero;
+    uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS] + one spare row
+    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 4u * SB_K * lane;
 
     sb_u64 acc[SB_D][SB_K / 2];
 #pragma unroll
@@ -362,10 +348,9 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const int nchan = c_end - c_begin;
     const int nstages = (nchan + CB - 1) / CB;
 
-    // Staging: warp w copies channel w of the stage (SB_CB == SB_WARPS); lane l copies logical chunks
-    // l, l+32, ... into the padded layout (sb_phys(l + 32 it) = sb_phys(l) + sb_phys(32) it). All of a warp's
-    // quantities but the lane term are warp-uniform; only windows that cross either end of the input
-    // allocation take the bounds-checked zero-filling path.
+    // Staging: warp w copies channel w of the stage (CB <= SB_WARPS) with one TMA bulk copy; only windows
+    // that cross either end of the input allocation take the bounds-checked zero-filling cp.async path
+    // (lane l copies chunks l, l+32, ...).
     const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sdata);
     const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
     // meta (window base, chunk count) of the channel this warp stages next: loaded one stage ahead so
@@ -386,25 +371,20 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         if (stage < nstages && cc < CB && c < c_end) {
             const int buf = stage % SB_STAGES;
             const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
-            const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes + 16u * sb_phys(lane);
-            const float *src = in + e0 + 4 * lane;
-            if (!SB_PADDED && e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
-                // plain layout, interior window: the whole window is one TMA bulk copy issued by one lane
+            const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes + 16u * lane;
+            if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
+                // interior window: the whole window is one TMA bulk copy issued by one lane
                 if (lane == 0) {
                     sb_mbar_expect_tx(full_bar, 16u * (unsigned)mt_cur.y);
                     sb_bulk_g2s(sdata_base + buf * stage_bytes + cc * slot_bytes, in + e0, 16u * (unsigned)mt_cur.y, full_bar);
                 }
-            } else if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
-#pragma unroll
-                for (int it = 0; it < SB_NCH_MAX / 32; ++it)
-                    if (lane + 32 * it < mt_cur.y) sb_cp_async16_s(dst + 16u * sb_phys(32) * it, src + 128 * it);
             } else {
                 for (int it = 0; it < SB_NCH_MAX / 32; ++it) {
                     if (lane + 32 * it >= mt_cur.y) break;
                     const long long e = e0 + 4 * lane + 128ll * it;
                     long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
                     valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
-                    sb_cp_async16_zs(dst + 16u * sb_phys(32) * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
+                    sb_cp_async16_zs(dst + 512u * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
                 }
             }
             if (lane < SB_WARPS / 2)   // the SB_WARPS records of this channel: contiguous, 16-byte aligned
@@ -423,7 +403,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 #define SB_DIST_CFG (SB_STAGES - 3)
 #endif
     constexpr int SB_DIST = SB_DIST_CFG;
-    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + SB_STAGES * CB * SB_WARPS);
+    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + (SB_STAGES * CB + 1) * SB_WARPS);   // after the spare record row
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
     if (tid == 0) {
 #pragma unroll
@@ -443,19 +423,10 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         sb_mbar_wait(bar_full + 8u * (stage % SB_STAGES), (unsigned)((stage / SB_STAGES) & 1));
         const int buf = stage % SB_STAGES;
         const int nch = min(CB, nchan - stage * CB);
-        const uint2 *recp = srec + (buf * CB) * SB_WARPS + warp;
-        unsigned slot_u32 = sdata_u32 + buf * stage_bytes;
-        uint2 rec_next = *recp;                            // record of channel ch+1 is fetched one channel ahead
-#pragma unroll 1
-        for (int ch = 0; ch < nch; ++ch, slot_u32 += slot_bytes) {
-            const uint2 rec = rec_next;                    // warp-uniform: x = SB_D 4-bit o_j, y = chunk base a
-            rec_next = recp[min(ch + 1, CB - 1) * SB_WARPS];
-            const unsigned obits = rec.x;
-            const unsigned ar = SB_PADDED ? rec.y & (unsigned)(SB_P - 1) : 0u;
-            const unsigned sa = slot_u32 + (SB_JOINT ? rec.y << 3 : (unsigned)sb_phys((int)rec.y) << 4);
-            (void)ar; (void)zero;
+        // the stage's channels, threaded: records are warp-uniform {x = pattern ids, y = window base in pairs}
+        const unsigned rp0 = (unsigned)__cvta_generic_to_shared(srec + (buf * CB) * SB_WARPS + warp);
+        const unsigned slot0 = sdata_u32 + buf * stage_bytes;
 #include "subband_rows.inc"
-        }
         __syncwarp();
         if (lane == 0) sb_mbar_arrive(bar_empty + 8u * (stage % SB_STAGES));
     }
@@ -657,10 +628,9 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     const int run_b0 = p->sb_blk_begin, run_b1 = p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end;   // caller's DM-block range
     A.blk0 = run_b0;
     A.nblk_run = run_b1 - run_b0;
-    A.slot_chunks = sb_phys(sb.max_nch) + 1;
-    A.zero = 0;
+    A.slot_chunks = sb.max_nch + 1;
     // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
-    auto ring_bytes = [&](int cb) { return (size_t)SB_STAGES * cb * A.slot_chunks * 16 + (size_t)SB_STAGES * cb * SB_WARPS * 8 + 16 * SB_STAGES; };
+    auto ring_bytes = [&](int cb) { return (size_t)SB_STAGES * cb * A.slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES; };
     A.cb = SB_CB;
     for (int cb = SB_CB_MAX; cb > SB_CB; cb -= 2)
         if (ring_bytes(cb) <= 227u * 1024u) { A.cb = cb; break; }

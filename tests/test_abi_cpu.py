@@ -111,19 +111,12 @@ def test_generated_channel_body_is_up_to_date():
     spec.loader.exec_module(gen)
     with open(os.path.join(csrc, "subband_rows.inc")) as f:
         committed = f.read()
-    tok = committed.splitlines()[0].split("gen_subband_rows.py")[1].split("-")[0].split()
+    d, k, sp, g, stride = (int(x) for x in committed.splitlines()[0].split("gen_subband_rows.py")[1].split("-")[0].split())
+    assert committed == gen.generate(d, k, sp, g, stride)
     with open(os.path.join(csrc, "plan.h")) as f:
         plan_h = f.read()
-    if tok[0] == "joint":
-        d, k, s, g = (int(x) for x in tok[1:5])
-        assert committed == gen.generate_joint(d, k, s, g)
-        assert "#define SB_JOINT_CFG 1" in plan_h and f"#define SB_D_CFG {d}" in plan_h
-        assert f"#define SB_K_CFG {k}" in plan_h and f"#define SB_S_CFG {s}" in plan_h and f"#define SB_G_CFG {g}" in plan_h
-    else:
-        d, k, omax, odd = (int(x) for x in tok[:4])
-        assert committed == gen.generate(d, k, omax, odd)
-        assert "#define SB_JOINT_CFG 0" in plan_h and f"#define SB_D_CFG {d}" in plan_h
-        assert f"#define SB_K_CFG {k}" in plan_h and f"#define SB_OMAX_CFG {omax}" in plan_h
+    assert f"#define SB_D_CFG {d}" in plan_h and f"#define SB_K_CFG {k}" in plan_h
+    assert f"#define SB_S_CFG {sp}" in plan_h and f"#define SB_G_CFG {g}" in plan_h
 
 
 def test_kernel_selection_falls_back_when_subband_is_not_admitted():
