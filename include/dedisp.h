@@ -147,6 +147,10 @@ long long dedisp_plan_verify_records(const dedisp_plan *plan);
 /* Number of kernel launches one dedisp_execute issues for this plan (for bench.py's gpu_launches). */
 int dedisp_plan_launches_per_execute(const dedisp_plan *plan);
 
+/* Number of DM slabs the last dedisp_execute_host call on this plan ran its final pass in (0: the
+ * call did not take the slab-overlap path). For the tests that must know which path they exercised. */
+int dedisp_plan_last_host_slabs(const dedisp_plan *plan);
+
 const char *dedisp_error_string(int code);
 const char *dedisp_last_cuda_error(const dedisp_plan *plan);
 

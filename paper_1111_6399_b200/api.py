@@ -30,7 +30,7 @@ SYMBOLS = (
     "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
-    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_error_string",
+    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_error_string",
     "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
@@ -62,7 +62,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_plan_max_shift.argtypes = [vp]
         L.dedisp_plan_max_shift.restype = c_ll
         for name in ("dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands",
-                     "dedisp_plan_launches_per_execute"):
+                     "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs"):
             getattr(L, name).argtypes = [vp]
         L.dedisp_plan_get_shifts.argtypes = [vp, ip]
         L.dedisp_plan_set_kernel.argtypes = [vp, c_int]
@@ -149,6 +149,10 @@ class Plan:
     @property
     def launches_per_execute(self) -> int:
         return int(lib().dedisp_plan_launches_per_execute(self._h))
+
+    @property
+    def last_host_slabs(self) -> int:
+        return int(lib().dedisp_plan_last_host_slabs(self._h))
 
     def num_subbands(self) -> int:
         return int(lib().dedisp_plan_num_subbands(self._h))

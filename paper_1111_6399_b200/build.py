@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)
-    flags = [f for f in NVCC_FLAGS if f not in ("-shared",)]
+    flags = [f for f in NVCC_FLAGS if f not in ("-shared",)] + os.environ.get("DEDISP_NVCC_EXTRA", "").split()
     for src in sources():
         obj = os.path.join(bdir, os.path.basename(src) + ".o")
         objs.append(obj)

@@ -23,7 +23,7 @@ int resolve_kernel(const dedisp_plan *p) {
 }  // namespace
 
 int execute_impl(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
-                 long long out_stride, Batch b, cudaStream_t st) {
+                 long long out_stride, Batch b, cudaStream_t st, const SbRun &run) {
     if (!p || !d_in || !d_out || nsamp_out < 1) return DEDISP_EINVAL;
     if (in_stride < nsamp_out + p->maxshift || out_stride < nsamp_out) return DEDISP_EINVAL;
     if (p->flags & DEDISP_PLAN_HOST_ONLY) return DEDISP_EUNSUPPORTED;
@@ -36,7 +36,7 @@ int execute_impl(dedisp_plan *p, const void *d_in, long long in_stride, long lon
     }
     cudaError_t e;
     switch (k) {
-        case DEDISP_KERNEL_SUBBAND: e = launch_subband(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
+        case DEDISP_KERNEL_SUBBAND: e = launch_subband(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st, run); break;
         case DEDISP_KERNEL_TILED: e = launch_tiled(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
         default: e = launch_naive(p, d_in, in_stride, nsamp_out, d_out, out_stride, b, st); break;
     }
@@ -151,7 +151,7 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
     // sub-bands in pass order on a second stream and let pass g start as soon as its rows have landed,
     // so that most of the H2D transfer hides under the earlier passes.
     const bool overlap = resolve_kernel(p) == DEDISP_KERNEL_SUBBAND && p->dtype == DEDISP_F32 && (nsamp_in & 3) == 0 &&
-                         p->sb.passes.size() > 1 && p->sb.nranges == 1;
+                         p->sb.passes.size() > 1 && p->sb.nranges == 1 && !subband_merges(p);   // a merged launch reads every channel at once
     if (overlap) {
         if (!p->host_copy_st) {
             e = cudaStreamCreateWithFlags(&p->host_copy_st, cudaStreamNonBlocking);
@@ -175,13 +175,17 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
             if (e == cudaSuccess) e = cudaEventRecord(p->host_pass_ready[g], p->host_copy_st);
         }
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
-        p->pass_ready = p->host_pass_ready.data();
-        p->sb_reverse = true;
     } else {
         e = cudaMemcpyAsync(p->d_host_in, h_in, in_bytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
     }
     int rc = DEDISP_OK;
+    SbRun run;
+    if (overlap) {
+        run.pass_ready = p->host_pass_ready.data();
+        run.reverse = true;
+    }
+    p->host_slabs = 0;
     if (overlap && p->sb.nblk >= 4) {
         // ... and run the LAST pass slab by slab over the DM blocks, so that the D2H copy of a finished
         // slab of out rows overlaps the rest of that pass
@@ -192,19 +196,20 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
             e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
             if (e == cudaSuccess) p->host_slab_done.push_back(ev);
         }
-        if (e != cudaSuccess) { p->pass_ready = nullptr; return fail_cuda(p, e, "dedisp_execute_host slabs"); }
+        if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host slabs");
         // all passes but the last over the whole grid, then the last pass slab by slab
         const int npass = (int)p->sb.passes.size();
-        p->sb_pass_lo = 0; p->sb_pass_hi = npass - 1;
-        rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
-        p->sb_pass_lo = npass - 1; p->sb_pass_hi = npass;
+        run.pass_lo = 0; run.pass_hi = npass - 1;
+        rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, run);
+        run.pass_lo = npass - 1; run.pass_hi = npass;
         for (int sl = 0; sl < NSLAB && rc == DEDISP_OK; ++sl) {
-            p->sb_blk_begin = (int)((long long)p->sb.nblk * sl / NSLAB);
-            p->sb_blk_end = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
-            rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
+            run.blk_lo = (int)((long long)p->sb.nblk * sl / NSLAB);
+            run.blk_hi = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
+            rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, run);
             if (rc != DEDISP_OK) break;
-            const long long d0 = std::min<long long>(p->ndm, (long long)p->sb_blk_begin * SB_ROWS);
-            const long long d1 = std::min<long long>(p->ndm, (long long)p->sb_blk_end * SB_ROWS);
+            ++p->host_slabs;
+            const long long d0 = std::min<long long>(p->ndm, (long long)run.blk_lo * SB_ROWS);
+            const long long d1 = std::min<long long>(p->ndm, (long long)run.blk_hi * SB_ROWS);
             e = cudaEventRecord(p->host_slab_done[sl], st);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_d2h_st, p->host_slab_done[sl], 0);
             if (e == cudaSuccess && d1 > d0)
@@ -212,17 +217,13 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
                                     (size_t)(d1 - d0) * nsamp_out * 4, cudaMemcpyDeviceToHost, p->host_d2h_st);
             if (e != cudaSuccess) rc = fail_cuda(p, e, "dedisp_execute_host slab D2H");
         }
-        p->sb_pass_lo = 0; p->sb_pass_hi = -1;
-        p->sb_blk_begin = 0; p->sb_blk_end = -1; p->pass_ready = nullptr; p->sb_reverse = false;
         if (rc != DEDISP_OK) return rc;
         e = cudaStreamSynchronize(p->host_d2h_st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host D2H");
         return DEDISP_OK;
     }
-    rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st);
-    p->pass_ready = nullptr;
-    p->sb_reverse = false;
+    rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, run);
     if (rc != DEDISP_OK) return rc;
     e = cudaMemcpyAsync(h_out, p->d_host_out, out_bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -297,6 +298,8 @@ long long dedisp_plan_verify_records(const dedisp_plan *p) {
     if (!p || !p->sb.ok) return -1;
     return subband_verify_records(p);
 }
+
+int dedisp_plan_last_host_slabs(const dedisp_plan *p) { return p ? p->host_slabs : -1; }
 
 int dedisp_plan_launches_per_execute(const dedisp_plan *p) {
     if (!p) return -1;

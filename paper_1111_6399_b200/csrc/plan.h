@@ -48,7 +48,7 @@ constexpr int SB_REC_STRIDE = SB_WARPS * 8;            // bytes between a warp's
 #endif
 constexpr int SB_CB = SB_CB_CFG;      // smallest number of channels per pipeline stage (one staging warp each)
 #ifndef SB_STAGES_CFG
-#define SB_STAGES_CFG 4
+#define SB_STAGES_CFG 2
 #endif
 constexpr int SB_STAGES = SB_STAGES_CFG;
 // staged 16-byte chunks per channel the slot can hold, a multiple of 32
@@ -61,23 +61,43 @@ struct SubbandPass {
     bool first = false;               // first pass of its DM range: stores instead of adding
 };
 
+// device copy of a pass (the kernel walks a range of these; nothing in it depends on nsamp_out)
+struct SbPassDev {
+    int c_begin, c_end;
+    int blk_begin, blk_end;
+    int max_skew;
+    int first;
+    int pad0, pad1;
+};
+
+// What one SUBBAND launch sequence covers: launch-order range of passes, DM-block range, order, and
+// (dedisp_execute_host) one "rows of pass g are on the device" event per pass. Passed by the caller;
+// the plan itself stays read-only during execute.
+struct SbRun {
+    int pass_lo = 0, pass_hi = -1;     // launch-order indices (-1: all)
+    int blk_lo = 0, blk_hi = -1;       // DM blocks (-1: all)
+    bool reverse = false;              // run the passes last sub-band first
+    const cudaEvent_t *pass_ready = nullptr;
+};
+
 struct SubbandGeom {
     bool ok = false;
     std::vector<SubbandPass> passes;
     int ngroups = 0, nblk = 0;
     int nranges = 0;                  // DM-block ranges, each with its own sub-band partition (1 for uniform DM plans)
-    // per (channel, group): low word = joint pattern ids, 8 bits per dispatch group (group 0 lowest):
+    // [nblk][nchans][SB_WARPS] per (block, channel, group): low word = joint pattern ids, 8 bits per dispatch group (group 0 lowest):
     // (o_a*(S+2) + o_b)..., high word = window base a in 8-byte pairs (subband.cu)
-    std::vector<uint64_t> records;    // [nchans][nblk*SB_WARPS]
-    // per (channel, block): {window base r (multiple of 4, relative to u), chunks to stage}
-    std::vector<int32_t> meta;        // [nchans][nblk][2]
+    std::vector<uint64_t> records;
+    // per (block, channel): {window base r (multiple of 4, relative to u), chunks to stage}
+    std::vector<int32_t> meta;        // [nblk][nchans][2]
     std::vector<int32_t> skew;        // [npasses][ndm] = s(c_ref(pass), d)
     uint64_t *d_records = nullptr;
     int32_t *d_meta = nullptr;
     int32_t *d_skew = nullptr;
-    int4 *d_ptab = nullptr;           // merged launch: per-pass {c_begin, c_end, pass, CTAs} for ptab_nsamp
-    long long ptab_nsamp = -1;
+    SbPassDev *d_passes = nullptr;    // [npasses]
     int max_nch = 0;                  // largest staged chunk count (sizes the shared-memory slot)
+    int slot_chunks = 0, cb = 0;      // launch geometry fixed at upload: slot size, channels per stage
+    size_t smem = 0;                  // dynamic shared memory of the kernel
 };
 
 struct dedisp_plan {
@@ -100,13 +120,10 @@ struct dedisp_plan {
     // dedisp_execute_host overlap: a copy stream and one "rows of pass g are on the device" event per pass
     cudaStream_t host_copy_st = nullptr;
     std::vector<cudaEvent_t> host_pass_ready;
-    const cudaEvent_t *pass_ready = nullptr;  // set only for the duration of one dedisp_execute_host call
     bool merge_fp_passes = false;             // fp plans: run all passes in one launch (sums not bit-reproducible)
-    bool sb_reverse = false;                  // run the passes last sub-band first (execute_host: smallest H2D first)
-    int sb_pass_lo = 0, sb_pass_hi = -1;      // launch-order range of passes the next SUBBAND launch runs (-1: all)
-    int sb_blk_begin = 0, sb_blk_end = -1;    // DM-block range the next SUBBAND launch covers (-1: all); execute_host slabs
     cudaStream_t host_d2h_st = nullptr;
     std::vector<cudaEvent_t> host_slab_done;
+    int host_slabs = 0;                       // DM slabs the last dedisp_execute_host call ran its last pass in (0: no slab overlap)
     // fp32 staging copy of the input for the SUBBAND kernel (u8/f16 input, or rows not 16-B aligned)
     float *d_conv = nullptr;
     size_t conv_bytes = 0;
@@ -139,9 +156,11 @@ void subband_free(dedisp_plan *p);
 long long subband_verify_records(const dedisp_plan *p);
 int subband_launches(const dedisp_plan *p, int resolved_kernel);  // kernel launches per execute
 cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams);  // staging-copy scratch
+bool subband_smem_fits(const dedisp_plan *p);
+bool subband_merges(const dedisp_plan *p);      // all passes of an execute in one launch?
 cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,
-                           void *d_out, long long out_stride, Batch b, cudaStream_t st);
+                           void *d_out, long long out_stride, Batch b, cudaStream_t st, const SbRun &run);
 
 // plan.cu (shared by the ABI entry points and stream.cu)
 int execute_impl(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
-                 long long out_stride, Batch b, cudaStream_t st);
+                 long long out_stride, Batch b, cudaStream_t st, const SbRun &run = SbRun());

@@ -82,15 +82,15 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
                         const uint32_t id = ((lo >> sh) & 255u) * (SB_S + 2) + (uint32_t)o;
                         lo = (lo & ~(255u << sh)) | (id << sh);
                     }
-                    p->sb.records[(size_t)c * gslots + q] = rec | lo;
+                    p->sb.records[((size_t)(q / SB_WARPS) * p->nchans + c) * SB_WARPS + q % SB_WARPS] = rec | lo;
                 }
             }
             // staged 16-byte chunks: the furthest lane of the furthest group must find its whole window
             const int nch = (2 * amax + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
             if (nch > SB_NCH_MAX || amax > 0xffff) return false;
             if (emit) {
-                p->sb.meta[((size_t)c * nblk + b) * 2 + 0] = rbase;
-                p->sb.meta[((size_t)c * nblk + b) * 2 + 1] = nch;
+                p->sb.meta[((size_t)b * p->nchans + c) * 2 + 0] = rbase;
+                p->sb.meta[((size_t)b * p->nchans + c) * 2 + 1] = nch;
                 p->sb.max_nch = std::max(p->sb.max_nch, nch);
             }
         }
@@ -192,8 +192,8 @@ void subband_build(dedisp_plan *p) {
         std::memcpy(sb.skew.data() + g * (size_t)ndm, sref, (size_t)ndm * sizeof(int32_t));
         ps.max_skew = sref[std::min(ndm, ps.blk_end * SB_ROWS) - 1];
     }
-    // the kernel's dynamic shared memory (ring + records) must fit the 227 KB a CTA may opt into
-    if ((size_t)SB_STAGES * SB_CB * ((size_t)(sb.max_nch + 1) * 16 + SB_REC_STRIDE + 16) + SB_REC_STRIDE > 227u * 1024u) { sb = SubbandGeom(); return; }
+    // the kernel's dynamic shared memory (ring + records + transpose buffers) must fit the 227 KB a CTA may opt into
+    if (!subband_smem_fits(p)) { sb = SubbandGeom(); return; }
     sb.ok = true;
 }
 
@@ -213,13 +213,13 @@ long long subband_verify_records(const dedisp_plan *p) {
             seen[c] += ps.blk_end - ps.blk_begin;
             for (int d = ps.blk_begin * SB_ROWS; d < std::min(ndm, ps.blk_end * SB_ROWS); ++d) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
-                const uint64_t rec = sb.records[(size_t)c * gslots + q];
+                const uint64_t rec = sb.records[((size_t)b * p->nchans + c) * SB_WARPS + q % SB_WARPS];
                 const int a = (int)((rec >> 32) & 0xffff);
                 uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
                 for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
                 const int o = (int)(id % (SB_S + 2));
-                const int rbase = sb.meta[((size_t)c * sb.nblk + b) * 2];
-                const int nch = sb.meta[((size_t)c * sb.nblk + b) * 2 + 1];
+                const int rbase = sb.meta[((size_t)b * p->nchans + c) * 2];
+                const int nch = sb.meta[((size_t)b * p->nchans + c) * 2 + 1];
                 const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 2 * a + o;
                 const int need = (2 * a + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
                 if (s != p->shifts[(size_t)c * ndm + d] || need > nch || (rbase & 3) || o > SB_OMAX) ++bad;
@@ -237,27 +237,34 @@ long long subband_verify_records(const dedisp_plan *p) {
 
 namespace {
 
-constexpr int SB_THREADS = SB_WARPS * 32;
-static_assert(SB_STAGES >= 4, "ring depth: prefetch distance SB_STAGES - 3 >= 1");
+// CTA = SB_WARPS consumer warps (three warpgroups, 160 registers each after setmaxnreg) + one producer
+// warpgroup (32 registers; its first warp issues every copy of the ring). Persistent: one CTA per SM
+// walks the launch's tiles round-robin, the producer streams the stages of consecutive tiles through
+// the ring back to back, and every consumer warp runs its own epilogue from a private transpose
+// buffer, so neither the ring fill of a tile nor its epilogue leaves the fp32 pipe idle. The ring is
+// only SB_STAGES = 2 deep on purpose: the consumer warps then never drift more than one stage apart,
+// which keeps the bodies they run hot in the instruction cache for each other (measured on c3: 4 stages
+// free-running 123.9 ms, 4 stages with a consumer barrier per stage 118.8, 2 stages free-running 111.1).
+constexpr int SB_CONSUMERS = SB_WARPS * 32;
+constexpr int SB_THREADS = SB_CONSUMERS + 128;
+constexpr int SB_REGS_CONSUMER = 160, SB_REGS_PRODUCER = 32;
+static_assert(SB_WARPS % 4 == 0, "setmaxnreg works on warpgroups");
+static_assert(SB_CONSUMERS * SB_REGS_CONSUMER + 128 * SB_REGS_PRODUCER <= 65536, "register file");
+static_assert(SB_STAGES >= 2, "ring depth");
 #ifndef SB_CB_MAX_CFG
-#define SB_CB_MAX_CFG SB_WARPS
+#define SB_CB_MAX_CFG 16
 #endif
-constexpr int SB_CB_MAX = SB_CB_MAX_CFG;
-static_assert(SB_CB_MAX <= SB_WARPS, "staging: at most one channel per warp and stage");   // channels per stage are chosen at launch (as many as fit)
-static_assert(SB_CB <= SB_WARPS, "the smallest stage: one channel per staging warp");
+constexpr int SB_CB_MAX = SB_CB_MAX_CFG;             // channels per stage are chosen at launch (as many as fit)
+static_assert(SB_CB_MAX <= 32 && SB_CB <= SB_CB_MAX, "one producer lane per staged channel");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
 // Staged layout: a channel's window is plain and contiguous (ONE TMA bulk copy); lanes are SB_K words
 // apart and SB_K/2 is odd, so LDS.64 is conflict-free (16 consecutive lanes hit 16 different bank pairs).
 static_assert(SB_K % 2 == 0 && (SB_K / 2) % 2 == 1, "K/2 odd: LDS.64 conflict-free in the plain layout");
-static_assert(SB_WARPS % 2 == 0 && SB_NCH_MAX % 32 == 0, "tile constants");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
 #undef SB_ROWS_PARAMS
 
-__device__ __forceinline__ void sb_cp_async16_s(unsigned sa, const void *gmem) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
-}
 __device__ __forceinline__ void sb_cp_async16_zs(unsigned sa, const void *gmem, int src_bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
 }
@@ -279,11 +286,15 @@ __device__ __forceinline__ void sb_mbar_arrive(unsigned bar) {
 __device__ __forceinline__ void sb_mbar_arrive_cp_async(unsigned bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
 }
+// producer side: the slot is usually still being read, so sleep instead of spinning on the issue slots
+// of the consumer warps that share this scheduler
+__device__ __forceinline__ void sb_mbar_wait_sleep(unsigned bar, unsigned parity) {
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1, %2;\n@p bra.uni DONE_%=;\nnanosleep.u32 256;\nbra.uni WAIT_%=;\nDONE_%=:\n}\n"
+                 ::"r"(bar), "r"(parity), "r"(100000u) : "memory");
+}
 __device__ __forceinline__ void sb_mbar_wait(unsigned bar, unsigned parity) {
     asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n@p bra.uni DONE_%=;\nbra.uni WAIT_%=;\nDONE_%=:\n}\n" ::"r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void sb_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void sb_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 struct SbArgs {
     const float *in;          // fp32 input, 16-byte aligned, stride % 4 == 0
@@ -293,202 +304,210 @@ struct SbArgs {
     void *out;
     long long out_stride, out_beam;
     long long nsamp_out;
-    const uint64_t *records;  // [nchans][gslots]
-    const int32_t *meta;      // [nchans][nblk][2]
-    const int32_t *skew;      // this pass: [ndm]
-    int c_begin, c_end;
-    int ndm, nblk, gslots;
-    int blk0, nblk_run;       // this launch covers DM blocks [blk0, blk0 + nblk_run)
-    int slot_chunks;          // physical 16-byte chunks per staged channel
+    const uint64_t *records;  // [nblk][nchans][SB_WARPS]
+    const int2 *meta;         // [nblk][nchans] {window base r relative to u (multiple of 4), 16-byte chunks to stage}
+    const int32_t *skew;      // [npasses][ndm]
+    const SbPassDev *passes;  // [npasses]
+    int pass_lo, pass_hi;     // this launch runs passes [pass_lo, pass_hi) of the table
+    int blk_lo, blk_hi;       // ... restricted to DM blocks [blk_lo, blk_hi)
+    int ndm, nchans, nbeams;
+    int slot_chunks;          // 16-byte chunks per staged channel slot
     int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
-    int first;                // 1: store, 0: add into out
-    const int4 *ptab;         // merged launch: per-pass {c_begin, c_end, pass index, CTAs}; skew = table of all passes
+    int first;                // 1: the launch's pass stores, 0: every pass adds into out
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
 };
 
-constexpr int SB_EP_PITCH = (SB_K / 2) % 2 == 1 ? SB_K + 4 : SB_K + 2;  // epilogue transpose: words per lane
-typedef unsigned long long sb_u64;  // one aligned register pair = two fp32 accumulators (FADD2 operand)
+constexpr int SB_EP_PITCH = SB_K + 4;  // epilogue transpose: words per lane, an odd number of 8-byte pairs
+typedef unsigned long long sb_u64;     // one aligned register pair = two fp32 accumulators (FADD2 operand)
 
-template <typename OutT, bool MERGED>
+// The CTA's next non-empty tile. Tiles of a pass are numbered beam-major, then u-tile, then DM block
+// (neighbouring CTAs work on neighbouring DM blocks of the same u-tile and share input windows in L2);
+// the tiles of all passes of the launch form one list dealt round-robin to the CTAs. The producer and
+// the consumers walk it with identical arithmetic.
+struct SbTile {
+    int p, w, rot;            // cursor: pass, next tile index of this CTA within it (-1: pass not opened), list offset mod grid
+    int blk, beam, c_begin, c_end;
+    long long U0;
+    const int32_t *skew;
+};
+
+__device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
+    const int grid = (int)gridDim.x;
+    for (;;) {
+        if (t.p >= A.pass_hi) return false;
+        const SbPassDev P = A.passes[t.p];
+        const int b0 = max(A.blk_lo, P.blk_begin), nb = min(A.blk_hi, P.blk_end) - b0;
+        const int ntu = (int)((A.nsamp_out + P.max_skew + SB_T - 1) / SB_T);
+        const int ntiles = nb > 0 ? A.nbeams * ntu * nb : 0;
+        if (t.w < 0) t.w = ((int)blockIdx.x + grid - t.rot) % grid;
+        if (t.w >= ntiles) { t.rot = (t.rot + ntiles % grid) % grid; ++t.p; t.w = -1; continue; }
+        const int w = t.w;
+        t.w += grid;
+        t.blk = b0 + w % nb;
+        const int rest = w / nb;
+        t.beam = rest / ntu;
+        t.U0 = (long long)(rest % ntu) * SB_T;
+        t.skew = A.skew + (size_t)t.p * A.ndm;
+        const int d_first = t.blk * SB_ROWS, d_last = min(A.ndm, d_first + SB_ROWS) - 1;
+        // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
+        if (t.U0 + SB_T <= (long long)__ldg(t.skew + d_first) || t.U0 >= (long long)__ldg(t.skew + d_last) + A.nsamp_out) continue;
+        t.c_begin = P.c_begin;
+        t.c_end = P.c_end;
+        return true;
+    }
+}
+
+template <typename OutT>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    // one pass per launch (ordered passes: deterministic fp32 sums), or all passes of the plan in one
-    // launch, pass = blockIdx.y (out zeroed beforehand, every pass adds with reductions: exact for u8 plans)
-    int c_begin = A.c_begin, c_end = A.c_end;
-    const int first = MERGED ? 0 : A.first;
-    const int32_t *skew = A.skew;
-    if constexpr (MERGED) {
-        const int4 pt = __ldg(A.ptab + blockIdx.y);      // {c_begin, c_end, pass index, CTAs of this pass}
-        if ((int)blockIdx.x >= pt.w) return;
-        c_begin = pt.x; c_end = pt.y;
-        skew = A.skew + (size_t)pt.z * A.ndm;
-    }
-    const int blk = A.blk0 + blockIdx.x % A.nblk_run;
-    const long long U0 = (long long)(blockIdx.x / A.nblk_run) * SB_T;
-    const int d_first = blk * SB_ROWS;
-    const int d_last = min(A.ndm, d_first + SB_ROWS) - 1;
-    // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
-    if (U0 + SB_T <= (long long)__ldg(skew + d_first) || U0 >= (long long)__ldg(skew + d_last) + A.nsamp_out) return;
-
-    const float *in = A.in + (size_t)blockIdx.z * A.in_beam;
     const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
     const int CB = A.cb;
     const unsigned stage_bytes = CB * slot_bytes;
-    unsigned char *sdata = sb_smem;                                             // [STAGES][CB][slot]
-    uint2 *srec = reinterpret_cast<uint2 *>(sb_smem + SB_STAGES * stage_bytes); // [STAGES][CB][WARPS] + one spare row
-    const unsigned sdata_u32 = (unsigned)__cvta_generic_to_shared(sdata) + 4u * SB_K * lane;
-
-    sb_u64 acc[SB_D][SB_K / 2];
-#pragma unroll
-    for (int j = 0; j < SB_D; ++j)
-#pragma unroll
-        for (int k = 0; k < SB_K / 2; ++k) acc[j][k] = 0ull;
-
-    const int nchan = c_end - c_begin;
-    const int nstages = (nchan + CB - 1) / CB;
-
-    // Staging: warp w copies channel w of the stage (CB <= SB_WARPS) with one TMA bulk copy; only windows
-    // that cross either end of the input allocation take the bounds-checked zero-filling cp.async path
-    // (lane l copies chunks l, l+32, ...).
-    const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sdata);
-    const int2 *meta2 = reinterpret_cast<const int2 *>(A.meta);
-    // meta (window base, chunk count) of the channel this warp stages next: loaded one stage ahead so
-    // that its L2 latency never sits in front of the copies
-    auto load_meta = [&](int stage) -> int2 {
-        const int cc = warp;
-        const int c = c_begin + stage * CB + cc;
-        if (stage < nstages && cc < CB && c < c_end) return __ldg(meta2 + (size_t)c * A.nblk + blk);
-        return make_int2(0, 0);
-    };
-    int2 mt = load_meta(0);
-    auto issue = [&](int stage, unsigned full_bar) {
-        {
-        const int cc = warp;                              // at most one channel per warp and stage (CB <= SB_WARPS)
-        const int c = c_begin + stage * CB + cc;
-        const int2 mt_cur = mt;
-        mt = load_meta(stage + 1);
-        if (stage < nstages && cc < CB && c < c_end) {
-            const int buf = stage % SB_STAGES;
-            const long long e0 = (long long)c * A.in_stride + U0 + mt_cur.x;
-            const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes + 16u * lane;
-            if (e0 >= 0 && e0 + 4ll * mt_cur.y <= A.in_total) {
-                // interior window: the whole window is one TMA bulk copy issued by one lane
-                if (lane == 0) {
-                    sb_mbar_expect_tx(full_bar, 16u * (unsigned)mt_cur.y);
-                    sb_bulk_g2s(sdata_base + buf * stage_bytes + cc * slot_bytes, in + e0, 16u * (unsigned)mt_cur.y, full_bar);
-                }
-            } else {
-                for (int it = 0; it < SB_NCH_MAX / 32; ++it) {
-                    if (lane + 32 * it >= mt_cur.y) break;
-                    const long long e = e0 + 4 * lane + 128ll * it;
-                    long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
-                    valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
-                    sb_cp_async16_zs(dst + 512u * it, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
-                }
-            }
-            if (lane < SB_WARPS / 2)   // the SB_WARPS records of this channel: contiguous, 16-byte aligned
-                sb_cp_async16_s((unsigned)__cvta_generic_to_shared(srec + (buf * CB + cc) * SB_WARPS) + 16u * lane,
-                                reinterpret_cast<const char *>(A.records + (size_t)c * A.gslots + blk * SB_WARPS) + 16 * lane);
-        }
-        }
-    };
-
-    // SB_STAGES-deep ring without CTA-wide barriers: full[b] completes when every thread's copies of
-    // the stage in buffer b have landed, empty[b] when every warp has finished reading it. A stage is
-    // refilled SB_DIST stages ahead, i.e. into the buffer read SB_STAGES - SB_DIST stages ago, so a
-    // fast warp can run SB_STAGES - SB_DIST - 1 whole stages ahead of the slowest before it has to wait
-    // (measured on c3: 4 stages, distance 1 => 170.8 ms; distance 2 => 172.2 ms).
-#ifndef SB_DIST_CFG
-#define SB_DIST_CFG (SB_STAGES - 3)
-#endif
-    constexpr int SB_DIST = SB_DIST_CFG;
-    const unsigned bar_full = (unsigned)__cvta_generic_to_shared(srec + (SB_STAGES * CB + 1) * SB_WARPS);   // after the spare record row
+    // [ring: STAGES x CB x slot][records: (STAGES x CB + 1) x SB_WARPS x 8][full, empty barriers][transpose buffers]
+    const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sb_smem);
+    const unsigned srec_base = sdata_base + SB_STAGES * stage_bytes;
+    const unsigned bar_full = srec_base + (SB_STAGES * CB + 1) * SB_REC_STRIDE;
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
     if (tid == 0) {
 #pragma unroll
-        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, SB_THREADS); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
+        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
     }
     __syncthreads();
-#pragma unroll
-    for (int st = 0; st < SB_DIST; ++st) { issue(st, bar_full + 8u * (st % SB_STAGES)); sb_mbar_arrive_cp_async(bar_full + 8u * (st % SB_STAGES)); }
-    for (int stage = 0; stage < nstages; ++stage) {
-        const int pst = stage + SB_DIST;
-        if (pst < nstages) {
-            const int pb = pst % SB_STAGES;
-            if (pst >= SB_STAGES) sb_mbar_wait(bar_empty + 8u * pb, (unsigned)((pst / SB_STAGES - 1) & 1));
-            issue(pst, bar_full + 8u * pb);
-            sb_mbar_arrive_cp_async(bar_full + 8u * pb);
-        }
-        sb_mbar_wait(bar_full + 8u * (stage % SB_STAGES), (unsigned)((stage / SB_STAGES) & 1));
-        const int buf = stage % SB_STAGES;
-        const int nch = min(CB, nchan - stage * CB);
-        // the stage's channels, threaded: records are warp-uniform {x = pattern ids, y = window base in pairs}
-        const unsigned rp0 = (unsigned)__cvta_generic_to_shared(srec + (buf * CB) * SB_WARPS + warp);
-        const unsigned slot0 = sdata_u32 + buf * stage_bytes;
-#include "subband_rows.inc"
-        __syncwarp();
-        if (lane == 0) sb_mbar_arrive(bar_empty + 8u * (stage % SB_STAGES));
-    }
+    SbTile t;
+    t.p = A.pass_lo; t.w = -1; t.rot = 0;
+    int it = 0;                                          // stages handed through the ring so far (all tiles)
 
-    // Epilogue: a lane holds SB_K consecutive samples of each row, so direct stores would touch 32
-    // sectors per instruction. Transpose through the (now idle) ring: each warp parks its tile in its
-    // own padded region and writes / read-modify-writes out[d][t] with lanes on consecutive samples.
-    __syncthreads();
-    constexpr int EP_PITCH = SB_EP_PITCH;                    // words per lane: an odd number of 8-byte pairs
-    float *ep = reinterpret_cast<float *>(sb_smem) + (size_t)warp * (SB_D * 32 * EP_PITCH);
-#pragma unroll
-    for (int j = 0; j < SB_D; ++j)
-#pragma unroll
-        for (int k2 = 0; k2 < SB_K / 2; ++k2)
-            *reinterpret_cast<sb_u64 *>(ep + (j * 32 + lane) * EP_PITCH + 2 * k2) = acc[j][k2];
-    __syncwarp();
-    OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)blockIdx.z * A.out_beam;
-#pragma unroll 1
-    for (int j = 0; j < SB_D; ++j) {
-        const int d = d_first + warp * SB_D + j;
-        if (d >= A.ndm) break;
-        const long long t0 = U0 - (long long)__ldg(skew + d);
-        OutT *orow = out + (size_t)d * A.out_stride;
-        const float *erow = ep + j * 32 * EP_PITCH;
-        auto E = [&](int sidx) { return erow[(sidx / SB_K) * EP_PITCH + (sidx % SB_K)]; };
-        auto put = [&](int sidx) {                           // one sample, bounds-checked
-            const long long t = t0 + sidx;
-            if (t >= 0 && t < A.nsamp_out) {
-                if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
-                    const int vi = __float2int_rn(E(sidx));
-                    orow[t] = first ? vi : orow[t] + vi;
-                } else {
-                    if (first) orow[t] = E(sidx);
-                    else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + t), "f"(E(sidx)) : "memory");
+    if (warp >= SB_WARPS) {
+        // ---------------- producer warpgroup: its first warp fills the ring
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(SB_REGS_PRODUCER));
+        if (warp != SB_WARPS) return;
+        while (sb_next_tile(A, t)) {
+            const float *in = A.in + (size_t)t.beam * A.in_beam;
+            const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
+            const uint64_t *recs = A.records + (size_t)t.blk * A.nchans * SB_WARPS;
+            for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {
+                const int buf = it % SB_STAGES, k = it / SB_STAGES;
+                const unsigned full = bar_full + 8u * buf;
+                if (k > 0) sb_mbar_wait_sleep(bar_empty + 8u * buf, (unsigned)((k - 1) & 1));
+                const int n = min(CB, t.c_end - c0);
+                // lane l stages channel c0 + l: an interior window is one TMA bulk copy
+                const bool mine = lane < n;
+                const int2 mt = mine ? __ldg(meta + c0 + lane) : make_int2(0, 0);
+                const long long e0 = (long long)(c0 + lane) * A.in_stride + t.U0 + mt.x;
+                const bool interior = e0 >= 0 && e0 + 4ll * mt.y <= A.in_total;
+                const unsigned dst = sdata_base + buf * stage_bytes + lane * slot_bytes;
+                if (mine && interior) {
+                    sb_mbar_expect_tx(full, 16u * (unsigned)mt.y);
+                    sb_bulk_g2s(dst, in + e0, 16u * (unsigned)mt.y, full);
                 }
-            }
-        };
-        if constexpr (std::is_floating_point<OutT>::value) {
-            if (A.out_vec4) {
-                // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
-                // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
-                const int m = (int)((-t0) & 3);              // samples before the first aligned t
-                const int nv = (SB_T - m) / 4;
-                for (int v = lane; v < nv; v += 32) {
-                    const int sidx = m + 4 * v;
-                    const long long t = t0 + sidx;
-                    if (t >= 0 && t + 3 < A.nsamp_out) {
-                        const float x0 = E(sidx), x1 = E(sidx + 1), x2 = E(sidx + 2), x3 = E(sidx + 3);
-                        if (first) *reinterpret_cast<float4 *>(orow + t) = make_float4(x0, x1, x2, x3);
-                        else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
-                                          ::"l"(orow + t), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
-                    } else {
-                        put(sidx); put(sidx + 1); put(sidx + 2); put(sidx + 3);
+                // windows that cross either end of the input allocation: bounds-checked zero-filling
+                // 16-byte cp.async by the whole warp, one such channel at a time
+                unsigned edge = __ballot_sync(0xffffffffu, mine && !interior);
+                while (edge) {
+                    const int cc = __ffs(edge) - 1;
+                    edge &= edge - 1;
+                    const long long e0c = __shfl_sync(0xffffffffu, e0, cc);
+                    const int nchc = __shfl_sync(0xffffffffu, mt.y, cc);
+                    const unsigned dstc = sdata_base + buf * stage_bytes + cc * slot_bytes;
+                    for (int ch = lane; ch < nchc; ch += 32) {
+                        const long long e = e0c + 4ll * ch;
+                        long long valid = e < 0 ? 0 : (A.in_total - e) * 4;
+                        valid = valid < 0 ? 0 : (valid > 16 ? 16 : valid);
+                        sb_cp_async16_zs(dstc + 16u * ch, valid ? (const void *)(in + e) : (const void *)in, (int)valid);
                     }
                 }
-                if (lane < m) put(lane);                                             // head
-                if (lane < SB_T - (m + 4 * nv)) put(m + 4 * nv + lane);              // tail
-                continue;
+                if (lane == 0) {   // the stage's records: n x SB_WARPS, contiguous
+                    sb_mbar_expect_tx(full, (unsigned)n * SB_REC_STRIDE);
+                    sb_bulk_g2s(srec_base + buf * CB * SB_REC_STRIDE, recs + (size_t)c0 * SB_WARPS, (unsigned)n * SB_REC_STRIDE, full);
+                }
+                sb_mbar_arrive_cp_async(full);
             }
         }
-#pragma unroll 8
-        for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
+        return;
+    }
+
+    // ---------------- consumer warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SB_REGS_CONSUMER));
+    const unsigned sdata_u32 = sdata_base + 4u * SB_K * lane;
+    const unsigned ep_off = (bar_empty + 8u * SB_STAGES - sdata_base + 15u) & ~15u;
+    float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * (32 * SB_EP_PITCH);
+    while (sb_next_tile(A, t)) {
+        sb_u64 acc[SB_D][SB_K / 2];
+#pragma unroll
+        for (int j = 0; j < SB_D; ++j)
+#pragma unroll
+            for (int k = 0; k < SB_K / 2; ++k) acc[j][k] = 0ull;
+
+        for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {
+            const int buf = it % SB_STAGES;
+            sb_mbar_wait(bar_full + 8u * buf, (unsigned)((it / SB_STAGES) & 1));
+            const int nch = min(CB, t.c_end - c0);
+            // the stage's channels, threaded: records are warp-uniform {x = pattern ids, y = window base in pairs}
+            const unsigned rp0 = srec_base + (buf * CB * SB_WARPS + warp) * 8u;
+            const unsigned slot0 = sdata_u32 + buf * stage_bytes;
+#include "subband_rows.inc"
+            __syncwarp();
+            if (lane == 0) sb_mbar_arrive(bar_empty + 8u * buf);
+        }
+
+        // Epilogue: a lane holds SB_K consecutive samples of each row, so direct stores would touch 32
+        // sectors per instruction. Each warp transposes row by row through its own buffer and writes /
+        // adds out[d][t] with lanes on consecutive 16-byte groups; no other warp is involved.
+        OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)t.beam * A.out_beam;
+        const int d0 = t.blk * SB_ROWS + warp * SB_D;
+        const int first = A.first;
+#pragma unroll
+        for (int j = 0; j < SB_D; ++j) {
+            const int d = d0 + j;
+            if (d >= A.ndm) break;
+            __syncwarp();
+#pragma unroll
+            for (int k2 = 0; k2 < SB_K / 2; ++k2)
+                *reinterpret_cast<sb_u64 *>(ep + lane * SB_EP_PITCH + 2 * k2) = acc[j][k2];
+            __syncwarp();
+            const long long t0 = t.U0 - (long long)__ldg(t.skew + d);
+            OutT *orow = out + (size_t)d * A.out_stride;
+            auto E = [&](int sidx) { return ep[(sidx / SB_K) * SB_EP_PITCH + (sidx % SB_K)]; };
+            auto put = [&](int sidx) {                           // one sample, bounds-checked
+                const long long tt = t0 + sidx;
+                if (tt >= 0 && tt < A.nsamp_out) {
+                    if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
+                        const int vi = __float2int_rn(E(sidx));
+                        orow[tt] = first ? vi : orow[tt] + vi;
+                    } else {
+                        if (first) orow[tt] = E(sidx);
+                        else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + tt), "f"(E(sidx)) : "memory");
+                    }
+                }
+            };
+            if constexpr (std::is_floating_point<OutT>::value) {
+                if (A.out_vec4) {
+                    // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
+                    // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
+                    const int m = (int)((-t0) & 3);              // samples before the first aligned t
+                    const int nv = (SB_T - m) / 4;
+#pragma unroll 1
+                    for (int v = lane; v < nv; v += 32) {
+                        const int sidx = m + 4 * v;
+                        const long long tt = t0 + sidx;
+                        if (tt >= 0 && tt + 3 < A.nsamp_out) {
+                            const float x0 = E(sidx), x1 = E(sidx + 1), x2 = E(sidx + 2), x3 = E(sidx + 3);
+                            if (first) *reinterpret_cast<float4 *>(orow + tt) = make_float4(x0, x1, x2, x3);
+                            else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
+                                              ::"l"(orow + tt), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
+                        } else {
+                            put(sidx); put(sidx + 1); put(sidx + 2); put(sidx + 3);
+                        }
+                    }
+                    if (lane < m) put(lane);                                             // head
+                    if (lane < SB_T - (m + 4 * nv)) put(m + 4 * nv + lane);              // tail
+                    continue;
+                }
+            }
+#pragma unroll 1
+            for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
+        }
     }
 }
 
@@ -517,6 +536,13 @@ __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__r
     *pv = __float2int_rn(__int_as_float(*pv));
 }
 
+// dynamic shared memory of the SUBBAND kernel for `cb` channels per stage
+size_t sb_smem_bytes(int cb, int slot_chunks) {
+    size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES;
+    b = (b + 15) / 16 * 16;
+    return b + (size_t)SB_WARPS * 32 * SB_EP_PITCH * sizeof(float);
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -525,44 +551,61 @@ __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__r
 cudaError_t subband_upload(dedisp_plan *p) {
     SubbandGeom &sb = p->sb;
     if (!sb.ok) return cudaSuccess;
+    std::vector<SbPassDev> tab(sb.passes.size());
+    for (size_t g = 0; g < sb.passes.size(); ++g) {
+        const SubbandPass &ps = sb.passes[g];
+        tab[g] = SbPassDev{ps.c_begin, ps.c_end, ps.blk_begin, ps.blk_end, ps.max_skew, ps.first ? 1 : 0, 0, 0};
+    }
     cudaError_t e = cudaMalloc(&sb.d_records, sb.records.size() * sizeof(uint64_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_records, sb.records.data(), sb.records.size() * sizeof(uint64_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&sb.d_meta, sb.meta.size() * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_meta, sb.meta.data(), sb.meta.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&sb.d_ptab, std::max<size_t>(1, sb.passes.size()) * sizeof(int4));
+    if (e == cudaSuccess) e = cudaMalloc(&sb.d_passes, tab.size() * sizeof(SbPassDev));
+    if (e == cudaSuccess) e = cudaMemcpy(sb.d_passes, tab.data(), tab.size() * sizeof(SbPassDev), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&sb.d_skew, sb.skew.size() * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_skew, sb.skew.data(), sb.skew.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
-    return e;
+    if (e != cudaSuccess) return e;
+    // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
+    sb.slot_chunks = sb.max_nch + 1;
+    sb.cb = SB_CB;
+    for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
+        if (sb_smem_bytes(cb, sb.slot_chunks) <= 227u * 1024u) { sb.cb = cb; break; }
+    sb.smem = sb_smem_bytes(sb.cb, sb.slot_chunks);
+    return cudaFuncSetAttribute(dedisp_subband_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
 }
 
 void subband_free(dedisp_plan *p) {
     if (p->sb.d_records) cudaFree(p->sb.d_records);
     if (p->sb.d_meta) cudaFree(p->sb.d_meta);
     if (p->sb.d_skew) cudaFree(p->sb.d_skew);
-    if (p->sb.d_ptab) cudaFree(p->sb.d_ptab);
-    p->sb.d_ptab = nullptr;
+    if (p->sb.d_passes) cudaFree(p->sb.d_passes);
     if (p->d_conv) cudaFree(p->d_conv);
     p->sb.d_records = nullptr;
     p->sb.d_meta = nullptr;
     p->sb.d_skew = nullptr;
+    p->sb.d_passes = nullptr;
     p->d_conv = nullptr;
     p->conv_bytes = 0;
 }
+
+bool subband_smem_fits(const dedisp_plan *p) { return sb_smem_bytes(SB_CB, p->sb.max_nch + 1) <= 227u * 1024u; }
 
 static bool sb_needs_staging_copy(const dedisp_plan *p, const void *d_in, long long in_stride, Batch b) {
     return p->dtype != DEDISP_F32 || ((uintptr_t)d_in & 15) != 0 || (in_stride & 3) != 0 || (b.n > 1 && (b.in_stride & 3) != 0);
 }
 
-// All passes in one launch? Measured (profiles/r1_paper_sweep.md): it pays only for plans cut into many
-// short passes (launch gaps and tile prologues dominate); long passes lose 2-5 % to idle CTAs and worse
-// L2 sharing. u8 plans (exact, order-independent sums) merge below 48 channels per pass on average;
-// fp plans only when the caller asked for it (dedisp_plan_set_pass_merge).
+// All passes in one launch? Ordered launches keep fp32 sums bit-reproducible (one add per address and
+// pass, in pass order) and cost a launch gap plus a drained machine per pass; that only matters for plans
+// cut into many short passes. u8 plans (exact, order-independent sums) merge below 48 channels per pass
+// on average; fp plans only when the caller asked for it (dedisp_plan_set_pass_merge).
 static bool sb_merge_passes(const dedisp_plan *p) {
     const size_t np = p->sb.passes.size();
-    if (np < 2) return false;
+    if (np < 2 || p->sb.nranges != 1) return false;
     if (p->dtype == DEDISP_U8) return (size_t)p->nchans <= 48 * np;
     return p->merge_fp_passes;
 }
+
+bool subband_merges(const dedisp_plan *p) { return sb_merge_passes(p); }
 
 int subband_launches(const dedisp_plan *p, int resolved_kernel) {
     if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
@@ -583,33 +626,40 @@ cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams) {
 }
 
 cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
-                           long long out_stride, Batch b, cudaStream_t st) {
+                           long long out_stride, Batch b, cudaStream_t st, const SbRun &run) {
     const SubbandGeom &sb = p->sb;
     const long long nsamp_in = nsamp_out + p->maxshift;
+    const int npass = (int)sb.passes.size();
+    const int pass_hi = run.pass_hi < 0 ? npass : run.pass_hi;
+    const int blk_lo = run.blk_lo, blk_hi = run.blk_hi < 0 ? sb.nblk : run.blk_hi;
+    const bool whole = run.pass_lo == 0 && pass_hi == npass && blk_lo == 0 && blk_hi == sb.nblk;
     SbArgs A;
     A.in = (const float *)d_in;
     A.in_stride = in_stride;
     A.in_total = (long long)(p->nchans - 1) * in_stride + nsamp_in;
     A.in_beam = b.in_stride;
+    cudaError_t e;
     if (sb_needs_staging_copy(p, d_in, in_stride, b)) {
         const long long pitch = (nsamp_in + 3) & ~3ll;
-        cudaError_t e = subband_reserve(p, nsamp_out, b.n);
-        if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)((nsamp_in + 255) / 256), (unsigned)p->nchans, (unsigned)b.n);
         const long long obeam = (long long)p->nchans * pitch;
-        switch (p->dtype) {
-            case DEDISP_U8:
-                dedisp_to_f32_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                break;
-            case DEDISP_F16:
-                dedisp_to_f32_kernel<__half><<<grid, 256, 0, st>>>((const __half *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                break;
-            default:
-                dedisp_to_f32_kernel<float><<<grid, 256, 0, st>>>((const float *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                break;
-        }
-        e = cudaGetLastError();
+        e = subband_reserve(p, nsamp_out, b.n);
         if (e != cudaSuccess) return e;
+        {
+            dim3 grid((unsigned)((nsamp_in + 255) / 256), (unsigned)p->nchans, (unsigned)b.n);
+            switch (p->dtype) {
+                case DEDISP_U8:
+                    dedisp_to_f32_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                    break;
+                case DEDISP_F16:
+                    dedisp_to_f32_kernel<__half><<<grid, 256, 0, st>>>((const __half *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                    break;
+                default:
+                    dedisp_to_f32_kernel<float><<<grid, 256, 0, st>>>((const float *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
+                    break;
+            }
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
         A.in = p->d_conv;
         A.in_stride = pitch;
         A.in_total = obeam;
@@ -621,80 +671,56 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.nsamp_out = nsamp_out;
     A.out_vec4 = ((uintptr_t)d_out & 15) == 0 && (out_stride & 3) == 0 && (b.n == 1 || (b.out_stride & 3) == 0);
     A.records = sb.d_records;
-    A.meta = sb.d_meta;
+    A.meta = reinterpret_cast<const int2 *>(sb.d_meta);
+    A.skew = sb.d_skew;
+    A.passes = sb.d_passes;
     A.ndm = p->ndm;
-    A.nblk = sb.nblk;
-    A.gslots = sb.nblk * SB_WARPS;
-    const int run_b0 = p->sb_blk_begin, run_b1 = p->sb_blk_end < 0 ? sb.nblk : p->sb_blk_end;   // caller's DM-block range
-    A.blk0 = run_b0;
-    A.nblk_run = run_b1 - run_b0;
-    A.slot_chunks = sb.max_nch + 1;
-    // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
-    auto ring_bytes = [&](int cb) { return (size_t)SB_STAGES * cb * A.slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES; };
-    A.cb = SB_CB;
-    for (int cb = SB_CB_MAX; cb > SB_CB; cb -= 2)
-        if (ring_bytes(cb) <= 227u * 1024u) { A.cb = cb; break; }
-    size_t smem = ring_bytes(A.cb);
-    smem = std::max(smem, (size_t)SB_WARPS * SB_D * 32 * SB_EP_PITCH * sizeof(float));  // epilogue transpose region
-    auto kern = dedisp_subband_kernel<float, false>;   // u8 plans too: fp32 sums in place, converted after the last pass
-    auto kern_merged = dedisp_subband_kernel<float, true>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern_merged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const size_t pass_hi = p->sb_pass_hi < 0 ? sb.passes.size() : (size_t)p->sb_pass_hi;
-    A.ptab = nullptr;
-    const bool whole = p->sb_pass_lo == 0 && pass_hi == sb.passes.size() && run_b0 == 0 && run_b1 == sb.nblk;
-    if (whole && sb.nranges == 1 && sb.d_ptab && sb_merge_passes(p)) {
-        // all passes in ONE launch (blockIdx.y = pass): out is zeroed, every pass adds with L2 reductions.
-        // Exact integers in fp32 are order-independent, so u8 plans stay bit-reproducible; fp plans only
-        // take this path when asked to (dedisp_plan_set_pass_merge), their sums then vary in the last bits.
+    A.nchans = p->nchans;
+    A.nbeams = b.n;
+    A.blk_lo = blk_lo;
+    A.blk_hi = blk_hi;
+    A.slot_chunks = sb.slot_chunks;
+    A.cb = sb.cb;
+    auto tiles_of = [&](const SubbandPass &ps) -> long long {
+        const long long nb = std::min(blk_hi, ps.blk_end) - std::max(blk_lo, ps.blk_begin);
+        return nb <= 0 ? 0 : nb * ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * b.n;
+    };
+    auto launch = [&](long long tiles) -> cudaError_t {
+        if (tiles <= 0) return cudaSuccess;
+        if (tiles >= (1ll << 31)) return cudaErrorInvalidValue;
+        const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, p->sm_count));
+        dedisp_subband_kernel<float><<<grid, SB_THREADS, sb.smem, st>>>(A);   // u8 plans too: fp32 sums in place, converted after the last pass
+        return cudaGetLastError();
+    };
+    if (whole && sb_merge_passes(p)) {
+        // all passes in ONE launch: out is zeroed, every pass adds with L2 reductions. Exact integers in
+        // fp32 are order-independent, so u8 plans stay bit-reproducible; fp plans only take this path when
+        // asked to (dedisp_plan_set_pass_merge), their sums then vary in the last bits.
         for (int bm = 0; bm < b.n; ++bm) {
             e = cudaMemset2DAsync((char *)d_out + (size_t)bm * b.out_stride * 4, (size_t)out_stride * 4, 0, (size_t)nsamp_out * 4, (size_t)p->ndm, st);
             if (e != cudaSuccess) return e;
         }
-        long long maxcta = 0;
-        for (const SubbandPass &ps : sb.passes) maxcta = std::max(maxcta, ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * sb.nblk);
-        std::vector<int4> tab(sb.passes.size());
-        for (size_t g = 0; g < sb.passes.size(); ++g)
-            tab[g] = make_int4(sb.passes[g].c_begin, sb.passes[g].c_end, (int)g, (int)(((nsamp_out + sb.passes[g].max_skew + SB_T - 1) / SB_T) * sb.nblk));
-        // the table depends on nsamp_out: refresh the device copy when it changed (stream-ordered)
-        if (sb.ptab_nsamp != nsamp_out) {
-            e = cudaMemcpyAsync(sb.d_ptab, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice, st);
-            if (e != cudaSuccess) return e;
-            e = cudaStreamSynchronize(st);   // tab is a local: the copy must finish before it goes away
-            if (e != cudaSuccess) return e;
-            p->sb.ptab_nsamp = nsamp_out;
-        }
-        A.ptab = sb.d_ptab;
-        A.skew = sb.d_skew;
-        A.c_begin = 0; A.c_end = 0; A.first = 0;
-        dim3 grid((unsigned)maxcta, (unsigned)sb.passes.size(), (unsigned)b.n);
-        kern_merged<<<grid, SB_THREADS, smem, st>>>(A);
-        e = cudaGetLastError();
+        long long tiles = 0;
+        for (const SubbandPass &ps : sb.passes) tiles += tiles_of(ps);
+        A.pass_lo = 0; A.pass_hi = npass; A.first = 0;
+        e = launch(tiles);
         if (e != cudaSuccess) return e;
-    } else
-    for (size_t i = (size_t)p->sb_pass_lo; i < pass_hi; ++i) {
-        const size_t g = p->sb_reverse ? sb.passes.size() - 1 - i : i;   // any order: the first launched pass stores
-        const SubbandPass &ps = sb.passes[g];
-        A.skew = sb.d_skew + g * (size_t)p->ndm;
-        A.c_begin = ps.c_begin;
-        A.c_end = ps.c_end;
-        A.blk0 = std::max(run_b0, ps.blk_begin);                     // the pass's DM range, clipped to the caller's
-        A.nblk_run = std::min(run_b1, ps.blk_end) - A.blk0;
-        if (A.nblk_run <= 0) continue;
-        A.first = sb.nranges == 1 ? i == 0 : ps.first;               // one range: any order, the first launched stores
-        const long long ntiles = (nsamp_out + ps.max_skew + SB_T - 1) / SB_T;
-        dim3 grid((unsigned)(ntiles * A.nblk_run), 1, (unsigned)b.n);
-        if (p->pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
-            e = cudaStreamWaitEvent(st, p->pass_ready[g], 0);
+    } else {
+        for (int i = run.pass_lo; i < pass_hi; ++i) {
+            const int g = run.reverse ? npass - 1 - i : i;
+            const SubbandPass &ps = sb.passes[g];
+            A.pass_lo = g; A.pass_hi = g + 1;
+            A.first = sb.nranges == 1 ? i == 0 : ps.first;   // one range: any order, the first launched pass stores
+            if (run.pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
+                e = cudaStreamWaitEvent(st, run.pass_ready[g], 0);
+                if (e != cudaSuccess) return e;
+            }
+            e = launch(tiles_of(ps));
             if (e != cudaSuccess) return e;
         }
-        kern<<<grid, SB_THREADS, smem, st>>>(A);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
     }
-    if (p->dtype == DEDISP_U8 && pass_hi == sb.passes.size()) {   // last pass done for these rows
-        const int d0 = std::min(p->ndm, run_b0 * SB_ROWS), d1 = std::min(p->ndm, run_b1 * SB_ROWS);
+    if (p->dtype == DEDISP_U8 && pass_hi == npass) {   // last pass done for these rows
+        const int d0 = std::min(p->ndm, blk_lo * SB_ROWS), d1 = std::min(p->ndm, blk_hi * SB_ROWS);
         for (int r0 = d0; r0 < d1; r0 += 32768) {   // grid.y <= 65535
             dim3 grid((unsigned)((nsamp_out + 255) / 256), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
             dedisp_f32_to_i32_inplace_kernel<<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
