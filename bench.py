@@ -107,8 +107,9 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def oracle_sample(cfg, target_s: float = 15.0):
-    """Time the oracle, as it stands, single-threaded, on a bounded row subset of the workload."""
+def oracle_sample(cfg, per_call_s: float = 3.0):
+    """The oracle, as it stands, on a bounded row subset of the workload: returns run(rows) -> seconds,
+    the row list sized for about per_call_s of one core, and the adds per row."""
     import numpy as np
     import oracle
     from paper_1111_6399_b200 import synth
@@ -117,30 +118,66 @@ def oracle_sample(cfg, target_s: float = 15.0):
     nsamp_in = cfg.nsamp_out + int(tab.max())
     x, _ = synth.make_input(cfg, tab, nsamp_in, device="cpu")
     x = x.numpy()
-    rate_guess = {"f32": 1.0e9, "u8": 2.0e9, "f16": 0.1e9}[cfg.dtype]
+    rate_guess = {"f32": 1.0e9, "u8": 2.0e9, "f16": 0.12e9}[cfg.dtype]
     per_row = cfg.nchans * cfg.nsamp_out
-    nrows = int(max(1, min(cfg.ndm, round(target_s * rate_guess / per_row))))
-    rows = np.linspace(0, cfg.ndm - 1, nrows).round().astype(np.int32)
+    nrows = int(max(1, min(cfg.ndm, round(per_call_s * rate_guess / per_row))))
 
-    def run():
+    def rows_for(n):
+        return np.linspace(0, cfg.ndm - 1, min(cfg.ndm, n)).round().astype(np.int32)
+
+    def run(rows):
         t0 = time.perf_counter()
         oracle.dedisperse(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, dm, x, cfg.nsamp_out, rows=rows)
         return time.perf_counter() - t0
 
-    return run, nrows * per_row, f"{nrows} of {cfg.ndm} DM rows (evenly spread) x all {cfg.nchans} channels x all " \
-                                 f"{cfg.nsamp_out} samples of {cfg.name}, single thread"
+    return run, rows_for, nrows, per_row
+
+
+def cpu_oracle_baseline(cfg, per_call_s: float = 3.0, repeats: int = 3):
+    """cpu_baseline: one warm-up call, then the median of `repeats` calls, (1) on one core and (2) on all
+    host cores - the unchanged single-threaded oracle entry point called on disjoint DM-row subsets from
+    one Python thread per core (ctypes releases the GIL), SURVEY.md section 8(d) "Oracle timing"."""
+    import numpy as np
+    from concurrent.futures import ThreadPoolExecutor
+    run, rows_for, nrows, per_row = oracle_sample(cfg, per_call_s)
+    rows = rows_for(nrows)
+    run(rows_for(1))                                     # warm-up: page in the input, build the oracle .so
+    t1 = sorted(run(rows) for _ in range(repeats))[repeats // 2]
+    cores = os.cpu_count() or 1
+    all_rows = rows_for(min(cfg.ndm, nrows * cores))
+    parts = [p for p in np.array_split(all_rows, cores) if p.size]
+
+    def run_all():
+        t0 = time.perf_counter()
+        with ThreadPoolExecutor(len(parts)) as ex:
+            list(ex.map(run, parts))
+        return time.perf_counter() - t0
+
+    run_all()
+    tn = sorted(run_all() for _ in range(repeats))[repeats // 2]
+    sample = (f"{rows.size} of {cfg.ndm} DM rows (evenly spread) x all {cfg.nchans} channels x all {cfg.nsamp_out} samples "
+              f"of {cfg.name}; 1 warm-up + median of {repeats} calls")
+    return {"value": rows.size * per_row / t1 / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+            "seconds_per_call": t1,
+            "all_cores": {"value": all_rows.size * per_row / tn / 1e9, "unit": UNIT, "cores": len(parts),
+                          "rows": int(all_rows.size), "seconds_per_call": tn,
+                          "how": "same oracle entry point, one Python thread per core on disjoint DM rows"}}
 
 
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    run, adds, sample = oracle_sample(cfg, target_s=8.0)
-    for _ in range(args.warmup):
-        run()
-    times = [run() for _ in range(args.steps)]
+    run, rows_for, nrows, per_row = oracle_sample(cfg, per_call_s=3.0)
+    rows = rows_for(nrows)
+    for _ in range(max(1, args.warmup)):
+        run(rows)
+    times = [run(rows) for _ in range(args.steps)]
     tot = sum(times)
+    adds = rows.size * per_row
     val = adds * args.steps / tot / 1e9
+    sample = (f"{rows.size} of {cfg.ndm} DM rows (evenly spread) x all {cfg.nchans} channels x all {cfg.nsamp_out} samples "
+              f"of {cfg.name}, single thread; each step = this sample")
     line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic", "impl": "reference",
@@ -152,9 +189,66 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per dedisp_execute from the committed ncu --set full
-# capture (profiles/), keyed by (workload, resolved kernel); None until captured.
-NCU_TRAFFIC_BYTES = {("c3_meerkat_f32", "subband"): 51.8e9}   # profiles/r1_subband.md: 26.7 GB read + 25.1 GB written per execute (12 passes)
+# dram__bytes_read.sum + dram__bytes_write.sum per dedisp_execute, summed over the launches of one
+# execute, from the committed ncu captures (profiles/r2_dram_<config>.csv), keyed by (workload, kernel)
+NCU_TRAFFIC_BYTES = {}
+_traffic_file = os.path.join(ROOT, "profiles", "r2_traffic.json")
+if os.path.exists(_traffic_file):
+    with open(_traffic_file) as _f:
+        NCU_TRAFFIC_BYTES = {tuple(k.split("/")): float(v) for k, v in json.load(_f).items()}
+
+
+def add_peak(sm_mhz: float) -> float:
+    return N_SM * LANES_PER_SM * sm_mhz * 1e6 / 1e9
+
+
+def resident_steps(plan, x, nsamp_out, out, steps, warmup):
+    """`steps` executes with the input resident in HBM, each bracketed by CUDA events on the launching
+    stream; returns the per-step device times (ms) and the time from the first to the last event."""
+    import torch
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        plan.execute(x, nsamp_out, out)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    torch.cuda.synchronize()
+    for a, b in evs:
+        a.record(stream)
+        plan.execute(x, nsamp_out, out)
+        b.record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs], evs[0][0].elapsed_time(evs[-1][1])
+
+
+def other_configs(sm_max_mhz: float, steps: int = 3, warmup: int = 3):
+    """The other full-size configs (c2, c4, c5-one-chunk-of-32-beams), resident inputs, a few steps each, so
+    that the driver-run default line records them too (they are parity-test cases, not the headline)."""
+    import torch
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import CONFIGS, synth
+    res = {}
+    for name in ("c2", "c4", "c5"):
+        cfg = CONFIGS[name]
+        plan = P.Plan.from_config(cfg)
+        nsamp_in = cfg.nsamp_out + plan.max_shift
+        tab = plan.shifts()
+        if cfg.nbeams > 1:
+            x = torch.empty((cfg.nbeams, cfg.nchans, nsamp_in), dtype=torch.uint8, device="cuda")
+            for b in range(cfg.nbeams):
+                x[b], _ = synth.make_input(cfg, tab, nsamp_in, device="cuda", seed=cfg.seed * 1000003 + b * 101)
+            out = plan.alloc_out(cfg.nsamp_out, cfg.nbeams)
+        else:
+            x, _ = synth.make_input(cfg, tab, nsamp_in, device="cuda")
+            out = plan.alloc_out(cfg.nsamp_out)
+        ms, _ = resident_steps(plan, x, cfg.nsamp_out, out, steps, warmup)
+        adds = cfg.nbeams * cfg.ndm * cfg.nchans * cfg.nsamp_out
+        med = sorted(ms)[len(ms) // 2]
+        kname = {1: "naive", 2: "tiled", 3: "subband"}[plan.kernel]
+        res[cfg.name] = {"ms_per_step": med, "value": adds / med / 1e6, "frac": adds / med / 1e6 / add_peak(sm_max_mhz),
+                         "kernel": kname, "launches_per_step": plan.launches_per_execute, "steps": steps,
+                         "beams": cfg.nbeams, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kname))}
+        del x, out, plan
+        torch.cuda.empty_cache()
+    return res
 
 
 def run_ours(args, cfg):
@@ -208,7 +302,8 @@ def run_ours(args, cfg):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     total_ms = max_over(evs[0][0].elapsed_time(evs[-1][1]))
-    step_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps       # device time of one execute
+    step_list = sorted(a.elapsed_time(b) for a, b in evs)
+    step_ms = sum(step_list) / args.steps                                # device time of one execute (mean)
     value = job_value(adds, args.steps, world, total_ms * 1e-3)
 
     # ---- e2e: the host-buffer C-ABI call; H2D + kernels + D2H inside the timed region
@@ -225,10 +320,25 @@ def run_ours(args, cfg):
             plan.execute_host(h_in, cfg.nsamp_out, h_out)
         barrier()
         et = max_over(time.perf_counter() - t0)
+        # outside the timed region: the host result of the LAST timed call against the device-resident
+        # `out` of the timed loop above (same input). The host call runs the passes in another order, so
+        # fp sums may differ in their last bits: |diff| <= 2e-5 * sum|terms| (each side within 1e-5 of the
+        # exact sum), with sum|terms| taken as nchans * mean|x|; integer outputs must be equal.
+        rows = torch.linspace(0, cfg.ndm - 1, min(cfg.ndm, 97)).round().long()
+        host_rows, dev_rows = h_out[rows], out[rows.cuda()].cpu()
+        if cfg.dtype == "u8":
+            e2e_ok, e2e_err = bool(torch.equal(host_rows, dev_rows)), 0.0
+        else:
+            bound = 2e-5 * cfg.nchans * float(x[:: max(1, cfg.nchans // 64)].float().abs().mean())
+            e2e_err = float((host_rows - dev_rows).abs().max())
+            e2e_ok = e2e_err <= bound
         e2e = {"value": job_value(adds, esteps, world, et), "unit": UNIT,
                "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
                "d2h_bytes_per_step": h_out.numel() * h_out.element_size(), "steps": esteps,
-               "ms_per_step": 1e3 * et / esteps, "api": "dedisp_execute_host (pinned host buffers)"}
+               "ms_per_step": 1e3 * et / esteps, "api": "dedisp_execute_host (pinned host buffers)",
+               "e2e_checked": e2e_ok, "e2e_check": f"{rows.numel()} rows of the last timed call's host output vs the "
+               f"device-resident output, max |diff| {e2e_err:.3g}", "host_slabs": plan.last_host_slabs}
+        assert e2e_ok, e2e["e2e_check"]
         del h_in, h_out
 
     if rank != 0:
@@ -236,7 +346,7 @@ def run_ours(args, cfg):
             dist.destroy_process_group()
         return
 
-    peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6 / 1e9            # Gadds/s at the max SM clock
+    peak = add_peak(sm_max_mhz)                                     # Gadds/s at the max SM clock
     achieved = adds / (step_ms * 1e-3) / 1e9
     esize = cfg.esize
     bytes_once = cfg.nchans * nsamp_in * esize + cfg.ndm * cfg.nsamp_out * 4
@@ -246,16 +356,22 @@ def run_ours(args, cfg):
                 "kernel": f"dedisp_{kname}_kernel", "launches_per_step": launches,
                 "peak_source": f"148 SMs x 128 lanes x sm_max_mhz ({peak_src} MEASURED_PEAKS.json clock)",
                 "hbm_bytes_once": bytes_once, "hbm_time_ms_at_peak": bytes_once / (hbm_gbs * 1e9) * 1e3,
-                "hbm_achieved_gbs": bytes_once / (step_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs}
+                "hbm_achieved_gbs": bytes_once / (step_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs,
+                "ms_mean": step_ms, "ms_median": step_list[len(step_list) // 2], "ms_best": step_list[0],
+                "frac_median": adds / (step_list[len(step_list) // 2] * 1e-3) / 1e9 / peak,
+                "frac_best": adds / (step_list[0] * 1e-3) / 1e9 / peak}
     if clocks and clocks.get("sm_mhz"):
-        roofline["frac_at_sampled_clock"] = achieved / (N_SM * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e9)
+        roofline["frac_at_sampled_clock"] = achieved / add_peak(clocks["sm_mhz"])
+
+    del x, out
+    torch.cuda.empty_cache()
+    others = None
+    if world == 1 and args.config == "c3" and not args.no_others and not args.kernel:
+        others = other_configs(sm_max_mhz)
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        run, sadds, sample = oracle_sample(cfg, target_s=args.cpu_seconds)
-        dt = run()
-        cpu_baseline = {"value": sadds / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                        "seconds": dt}
+        cpu_baseline = cpu_oracle_baseline(cfg, per_call_s=args.cpu_seconds)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -267,7 +383,7 @@ def run_ours(args, cfg):
                        "parallelism": f"{world} independent beams, one per GPU, no collective"},
             "real_time_factor": cfg.nsamp_out * cfg.tsamp / (total_ms / args.steps * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches * args.steps,
-            "roofline": roofline, "cpu_baseline": cpu_baseline}
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "others": others}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -406,7 +522,8 @@ def main():
     ap.add_argument("--kernel", default=None, choices=["naive", "tiled", "subband"])
     ap.add_argument("--merge-passes", action="store_true", help="fp plans: all SUBBAND passes in one launch (not bit-reproducible)")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--cpu-seconds", type=float, default=3.0, help="cpu_baseline: oracle seconds per timed call")
+    ap.add_argument("--no-others", action="store_true", help="skip the c2/c4/c5 block of the default line")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -29,8 +29,8 @@ int execute_impl(dedisp_plan *p, const void *d_in, long long in_stride, long lon
     if (p->flags & DEDISP_PLAN_HOST_ONLY) return DEDISP_EUNSUPPORTED;
     if (nsamp_out + p->maxshift >= (1ll << 40)) return DEDISP_EUNSUPPORTED;
     int k = resolve_kernel(p);
-    // the staged kernels align window starts down to 16 B relative to an aligned base
-    if (((uintptr_t)d_in & 15) != 0 && k != DEDISP_KERNEL_NAIVE) {
+    // TILED aligns window starts down to 16 B relative to an aligned base (SUBBAND takes any alignment)
+    if (((uintptr_t)d_in & 15) != 0 && k == DEDISP_KERNEL_TILED) {
         if (p->kernel != DEDISP_KERNEL_AUTO) return DEDISP_EINVAL;
         k = DEDISP_KERNEL_NAIVE;
     }

@@ -98,6 +98,8 @@ struct SubbandGeom {
     int max_nch = 0;                  // largest staged chunk count (sizes the shared-memory slot)
     int slot_chunks = 0, cb = 0;      // launch geometry fixed at upload: slot size, channels per stage
     size_t smem = 0;                  // dynamic shared memory of the kernel
+    int raw_slot_bytes = 0, cb_raw = 0;   // the same for the raw path (u8 / f16 input, unaligned fp32 rows)
+    size_t smem_raw = 0;
 };
 
 struct dedisp_plan {
@@ -124,9 +126,6 @@ struct dedisp_plan {
     cudaStream_t host_d2h_st = nullptr;
     std::vector<cudaEvent_t> host_slab_done;
     int host_slabs = 0;                       // DM slabs the last dedisp_execute_host call ran its last pass in (0: no slab overlap)
-    // fp32 staging copy of the input for the SUBBAND kernel (u8/f16 input, or rows not 16-B aligned)
-    float *d_conv = nullptr;
-    size_t conv_bytes = 0;
 };
 
 inline int dtype_esize(int dtype) { return dtype == DEDISP_U8 ? 1 : dtype == DEDISP_F16 ? 2 : 4; }
@@ -155,7 +154,6 @@ cudaError_t subband_upload(dedisp_plan *p);
 void subband_free(dedisp_plan *p);
 long long subband_verify_records(const dedisp_plan *p);
 int subband_launches(const dedisp_plan *p, int resolved_kernel);  // kernel launches per execute
-cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams);  // staging-copy scratch
 bool subband_smem_fits(const dedisp_plan *p);
 bool subband_merges(const dedisp_plan *p);      // all passes of an execute in one launch?
 cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,

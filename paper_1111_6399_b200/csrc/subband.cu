@@ -247,9 +247,12 @@ namespace {
 // free-running 123.9 ms, 4 stages with a consumer barrier per stage 118.8, 2 stages free-running 111.1).
 constexpr int SB_CONSUMERS = SB_WARPS * 32;
 constexpr int SB_THREADS = SB_CONSUMERS + 128;
-constexpr int SB_REGS_CONSUMER = 160, SB_REGS_PRODUCER = 32;
-static_assert(SB_WARPS % 4 == 0, "setmaxnreg works on warpgroups");
-static_assert(SB_CONSUMERS * SB_REGS_CONSUMER + 128 * SB_REGS_PRODUCER <= 65536, "register file");
+// registers per thread after setmaxnreg: the direct fp32 kernel's producer only issues copies (32 are
+// plenty); the raw path's producer warps convert, and with 32 registers their loop spilled to local
+// memory, which has no L1 to speak of next to 200+ KB of shared memory (c5: 83.0 ms -> 77.3 ms with 56)
+template <bool RAW> struct SbRegs { static constexpr int consumer = RAW ? 152 : 160, producer = RAW ? 56 : 32; };
+static_assert(SB_CONSUMERS * SbRegs<false>::consumer + 128 * SbRegs<false>::producer <= 65536, "register file");
+static_assert(SB_CONSUMERS * SbRegs<true>::consumer + 128 * SbRegs<true>::producer <= 65536, "register file");
 static_assert(SB_STAGES >= 2, "ring depth");
 #ifndef SB_CB_MAX_CFG
 #define SB_CB_MAX_CFG 16
@@ -297,7 +300,7 @@ __device__ __forceinline__ void sb_mbar_wait(unsigned bar, unsigned parity) {
 }
 
 struct SbArgs {
-    const float *in;          // fp32 input, 16-byte aligned, stride % 4 == 0
+    const void *in;           // direct path: fp32, 16-byte aligned, strides % 4 == 0; raw path: any dtype / alignment
     long long in_stride;      // elements
     long long in_total;       // readable elements per beam starting at `in`
     long long in_beam;        // elements between beams
@@ -312,6 +315,7 @@ struct SbArgs {
     int blk_lo, blk_hi;       // ... restricted to DM blocks [blk_lo, blk_hi)
     int ndm, nchans, nbeams;
     int slot_chunks;          // 16-byte chunks per staged channel slot
+    int raw_slot_bytes;       // raw path: bytes per raw channel slot
     int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
     int first;                // 1: the launch's pass stores, 0: every pass adds into out
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
@@ -357,21 +361,53 @@ __device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
     }
 }
 
-template <typename OutT>
+// four fp32 samples from a raw staged window (shared memory, element type TIN) at byte offset `off`
+template <typename TIN>
+__device__ __forceinline__ float4 sb_raw4(unsigned raw_u32, unsigned off) {
+    const unsigned wa = raw_u32 + (off & ~3u), sh = (off & 3u) * 8u;
+    auto lds = [](unsigned a) { unsigned v; asm volatile("ld.shared.b32 %0, [%1];\n" : "=r"(v) : "r"(a)); return v; };
+    if constexpr (std::is_same<TIN, uint8_t>::value) {
+        const unsigned v = __funnelshift_r(lds(wa), lds(wa + 4), sh);
+        return make_float4((float)(v & 255u), (float)((v >> 8) & 255u), (float)((v >> 16) & 255u), (float)(v >> 24));
+    } else if constexpr (std::is_same<TIN, __half>::value) {
+        const unsigned w0 = lds(wa), w1 = lds(wa + 4), w2 = lds(wa + 8);
+        const unsigned a = __funnelshift_r(w0, w1, sh), b = __funnelshift_r(w1, w2, sh);
+        const float2 fa = __half22float2(*reinterpret_cast<const __half2 *>(&a)), fb = __half22float2(*reinterpret_cast<const __half2 *>(&b));
+        return make_float4(fa.x, fa.y, fb.x, fb.y);
+    } else {
+        return make_float4(__uint_as_float(lds(wa)), __uint_as_float(lds(wa + 4)), __uint_as_float(lds(wa + 8)), __uint_as_float(lds(wa + 12)));
+    }
+}
+template <typename TIN> __device__ __forceinline__ float sb_to_f32(TIN v) { return (float)v; }
+template <> __device__ __forceinline__ float sb_to_f32<__half>(__half v) { return __half2float(v); }
+
+// TIN = input element type. RAW = false: fp32 rows whose base and pitches are 16-byte aligned are copied
+// by TMA straight into the ring. RAW = true (u8 / f16 input, or fp32 rows of any alignment): the
+// windows are TMA-copied as raw bytes (from the 16-byte boundary below their first sample) into a raw
+// buffer, and the four producer warps convert them to fp32 into the ring - no pre-pass over the input
+// and no fp32 copy of it in HBM.
+template <typename TIN, bool RAW>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
+    typedef float OutT;
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
     const int CB = A.cb;
     const unsigned stage_bytes = CB * slot_bytes;
-    // [ring: STAGES x CB x slot][records: (STAGES x CB + 1) x SB_WARPS x 8][full, empty barriers][transpose buffers]
+    // [ring: STAGES x CB x slot][records: (STAGES x CB + 1) x SB_WARPS x 8][full, empty, raw_full, raw_empty barriers]
+    // [transpose buffers][raw: CB x raw_slot]
     const unsigned sdata_base = (unsigned)__cvta_generic_to_shared(sb_smem);
     const unsigned srec_base = sdata_base + SB_STAGES * stage_bytes;
     const unsigned bar_full = srec_base + (SB_STAGES * CB + 1) * SB_REC_STRIDE;
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
+    const unsigned bar_raw_full = bar_empty + 8u * SB_STAGES, bar_raw_empty = bar_raw_full + 8u;
+    const unsigned ep_off = (bar_raw_empty + 8u - sdata_base + 15u) & ~15u;
+    const unsigned raw_base = sdata_base + ep_off + SB_WARPS * 32 * SB_EP_PITCH * 4;
     if (tid == 0) {
 #pragma unroll
-        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
+        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, RAW ? 4 : 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
+        sb_mbar_init(bar_raw_full, 1);
+        sb_mbar_init(bar_raw_empty, 4);
     }
     __syncthreads();
     SbTile t;
@@ -380,10 +416,80 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 
     if (warp >= SB_WARPS) {
         // ---------------- producer warpgroup: its first warp fills the ring
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(SB_REGS_PRODUCER));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(SbRegs<RAW>::producer));
+        if constexpr (RAW) {
+            const int pw = warp - SB_WARPS;
+            constexpr long long ES = (long long)sizeof(TIN);
+            const long long in_bytes = A.in_total * ES;
+            while (sb_next_tile(A, t)) {
+                const char *inb = reinterpret_cast<const char *>(A.in) + (size_t)t.beam * A.in_beam * ES;
+                const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
+                for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {
+                    const int buf = it % SB_STAGES, k = it / SB_STAGES;
+                    const unsigned full = bar_full + 8u * buf;
+                    const int n = min(CB, t.c_end - c0);
+                    // window of channel c: samples [e0, e0 + 4 nch); raw bytes from the 16-byte boundary at or below
+                    // its first sample (lead bytes in front). A window whose raw copy would leave the beam's byte
+                    // range is not copied at all: its converter reads global memory with bounds checks.
+                    auto window = [&](int c, long long &g, unsigned &lead, unsigned &rb, int &nch) -> bool {
+                        const int2 mt = __ldg(meta + c);
+                        nch = mt.y;
+                        g = ((long long)c * A.in_stride + t.U0 + mt.x) * ES;
+                        lead = (unsigned)((reinterpret_cast<uintptr_t>(inb) + (unsigned long long)g) & 15u);
+                        rb = (lead + 4u * (unsigned)mt.y * (unsigned)ES + 15u) & ~15u;
+                        return g - lead >= 0 && g - lead + rb <= in_bytes;
+                    };
+                    if (pw == 0) {   // copy warp: lane l copies the raw window of channel c0 + l with one TMA bulk copy
+                        if (it > 0) sb_mbar_wait_sleep(bar_raw_empty, (unsigned)((it - 1) & 1));
+                        if (lane < n) {
+                            long long g; unsigned lead, rb; int nch;
+                            if (window(c0 + lane, g, lead, rb, nch)) {
+                                sb_mbar_expect_tx(bar_raw_full, rb);
+                                sb_bulk_g2s(raw_base + lane * (unsigned)A.raw_slot_bytes, inb + (g - lead), rb, bar_raw_full);
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) sb_mbar_arrive(bar_raw_full);
+                    }
+                    if (k > 0) sb_mbar_wait_sleep(bar_empty + 8u * buf, (unsigned)((k - 1) & 1));
+                    if (pw == 0 && lane == 0) {   // the stage's records: n x SB_WARPS, contiguous
+                        sb_mbar_expect_tx(full, (unsigned)n * SB_REC_STRIDE);
+                        sb_bulk_g2s(srec_base + buf * CB * SB_REC_STRIDE, A.records + ((size_t)t.blk * A.nchans + c0) * SB_WARPS, (unsigned)n * SB_REC_STRIDE, full);
+                    }
+                    sb_mbar_wait(bar_raw_full, (unsigned)(it & 1));
+                    for (int cc = pw; cc < n; cc += 4) {   // this warp converts channels pw, pw + 4, ... of the stage
+                        long long g; unsigned lead, rb; int nch;
+                        const bool interior = window(c0 + cc, g, lead, rb, nch);
+                        const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes;
+                        if (interior) {
+                            const unsigned raw = raw_base + cc * (unsigned)A.raw_slot_bytes;
+                            for (int i = lane; i < nch; i += 32) {
+                                const float4 v = sb_raw4<TIN>(raw, lead + 4u * (unsigned)ES * i);
+                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n" ::"r"(dst + 16u * i), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+                            }
+                        } else {
+                            const TIN *src = reinterpret_cast<const TIN *>(inb);
+                            const long long e0 = g / ES;
+                            for (int i = lane; i < nch; i += 32) {
+                                float v[4];
+#pragma unroll
+                                for (int q = 0; q < 4; ++q) {
+                                    const long long e = e0 + 4 * i + q;
+                                    v[q] = e >= 0 && e < A.in_total ? sb_to_f32<TIN>(src[e]) : 0.f;
+                                }
+                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n" ::"r"(dst + 16u * i), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) { sb_mbar_arrive(full); sb_mbar_arrive(bar_raw_empty); }
+                }
+            }
+            return;
+        }
         if (warp != SB_WARPS) return;
         while (sb_next_tile(A, t)) {
-            const float *in = A.in + (size_t)t.beam * A.in_beam;
+            const float *in = reinterpret_cast<const float *>(A.in) + (size_t)t.beam * A.in_beam;
             const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
             const uint64_t *recs = A.records + (size_t)t.blk * A.nchans * SB_WARPS;
             for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {
@@ -428,9 +534,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     }
 
     // ---------------- consumer warps
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SB_REGS_CONSUMER));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SbRegs<RAW>::consumer));
     const unsigned sdata_u32 = sdata_base + 4u * SB_K * lane;
-    const unsigned ep_off = (bar_empty + 8u * SB_STAGES - sdata_base + 15u) & ~15u;
     float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * (32 * SB_EP_PITCH);
     while (sb_next_tile(A, t)) {
         sb_u64 acc[SB_D][SB_K / 2];
@@ -511,21 +616,6 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     }
 }
 
-// input staging copy: any dtype / any stride -> fp32 rows with a 16-byte-aligned pitch
-template <typename TIN>
-__global__ void __launch_bounds__(256) dedisp_to_f32_kernel(const TIN *__restrict__ in, long long in_stride, long long in_beam,
-                                                            float *__restrict__ out, long long out_stride, long long out_beam,
-                                                            long long ncols) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= ncols) return;
-    const TIN *src = in + (size_t)blockIdx.z * in_beam + (size_t)blockIdx.y * in_stride;
-    float *dst = out + (size_t)blockIdx.z * out_beam + (size_t)blockIdx.y * out_stride;
-    float v;
-    if constexpr (std::is_same<TIN, __half>::value) v = __half2float(src[i]);
-    else v = (float)src[i];
-    dst[i] = v;
-}
-
 // u8 plans: the passes accumulate exact fp32 sums in place in the caller's int32 buffer (so that every
 // pass can use the vector reduction); this turns the finished rows into int32, in place.
 __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__restrict__ out, long long out_stride, long long out_beam,
@@ -536,11 +626,17 @@ __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__r
     *pv = __float2int_rn(__int_as_float(*pv));
 }
 
-// dynamic shared memory of the SUBBAND kernel for `cb` channels per stage
-size_t sb_smem_bytes(int cb, int slot_chunks) {
-    size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES;
+// raw path: bytes per raw channel slot (window bytes + up to 15 lead bytes, rounded up to 16, + one
+// spare chunk the realigning loads may touch)
+int sb_raw_slot_bytes(int slot_chunks, int esize) { return ((slot_chunks * 4 * esize + 15 + 15) & ~15) + 16; }
+
+// dynamic shared memory of the SUBBAND kernel for `cb` channels per stage (esize > 0: raw path)
+size_t sb_smem_bytes(int cb, int slot_chunks, int esize) {
+    size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES + 16;
     b = (b + 15) / 16 * 16;
-    return b + (size_t)SB_WARPS * 32 * SB_EP_PITCH * sizeof(float);
+    b += (size_t)SB_WARPS * 32 * SB_EP_PITCH * sizeof(float);
+    if (esize > 0) b += (size_t)cb * sb_raw_slot_bytes(slot_chunks, esize);
+    return b;
 }
 
 }  // namespace
@@ -567,11 +663,24 @@ cudaError_t subband_upload(dedisp_plan *p) {
     if (e != cudaSuccess) return e;
     // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
     sb.slot_chunks = sb.max_nch + 1;
-    sb.cb = SB_CB;
-    for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
-        if (sb_smem_bytes(cb, sb.slot_chunks) <= 227u * 1024u) { sb.cb = cb; break; }
-    sb.smem = sb_smem_bytes(sb.cb, sb.slot_chunks);
-    return cudaFuncSetAttribute(dedisp_subband_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+    const int esize = dtype_esize(p->dtype);
+    sb.raw_slot_bytes = sb_raw_slot_bytes(sb.slot_chunks, esize);
+    auto pick = [&](int es, int &cb_out, size_t &smem_out) {
+        cb_out = SB_CB;
+        for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
+            if (sb_smem_bytes(cb, sb.slot_chunks, es) <= 227u * 1024u) { cb_out = cb; break; }
+        smem_out = sb_smem_bytes(cb_out, sb.slot_chunks, es);
+    };
+    pick(0, sb.cb, sb.smem);
+    pick(esize, sb.cb_raw, sb.smem_raw);
+    switch (p->dtype) {
+        case DEDISP_U8: return cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+        case DEDISP_F16: return cudaFuncSetAttribute(dedisp_subband_kernel<__half, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+        default: break;
+    }
+    e = cudaFuncSetAttribute(dedisp_subband_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+    return e;
 }
 
 void subband_free(dedisp_plan *p) {
@@ -579,18 +688,17 @@ void subband_free(dedisp_plan *p) {
     if (p->sb.d_meta) cudaFree(p->sb.d_meta);
     if (p->sb.d_skew) cudaFree(p->sb.d_skew);
     if (p->sb.d_passes) cudaFree(p->sb.d_passes);
-    if (p->d_conv) cudaFree(p->d_conv);
     p->sb.d_records = nullptr;
     p->sb.d_meta = nullptr;
     p->sb.d_skew = nullptr;
     p->sb.d_passes = nullptr;
-    p->d_conv = nullptr;
-    p->conv_bytes = 0;
 }
 
-bool subband_smem_fits(const dedisp_plan *p) { return sb_smem_bytes(SB_CB, p->sb.max_nch + 1) <= 227u * 1024u; }
+bool subband_smem_fits(const dedisp_plan *p) { return sb_smem_bytes(SB_CB, p->sb.max_nch + 1, dtype_esize(p->dtype)) <= 227u * 1024u; }
 
-static bool sb_needs_staging_copy(const dedisp_plan *p, const void *d_in, long long in_stride, Batch b) {
+// fp32 rows whose base and pitches are 16-byte aligned go straight into the ring; everything else takes the
+// raw path (TMA of the raw bytes + conversion / realignment by the producer warps)
+static bool sb_raw_path(const dedisp_plan *p, const void *d_in, long long in_stride, Batch b) {
     return p->dtype != DEDISP_F32 || ((uintptr_t)d_in & 15) != 0 || (in_stride & 3) != 0 || (b.n > 1 && (b.in_stride & 3) != 0);
 }
 
@@ -610,19 +718,7 @@ bool subband_merges(const dedisp_plan *p) { return sb_merge_passes(p); }
 int subband_launches(const dedisp_plan *p, int resolved_kernel) {
     if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
     const bool merged = sb_merge_passes(p);   // + a memset, which is not a kernel
-    return (merged ? 1 : (int)p->sb.passes.size()) + (p->dtype != DEDISP_F32 ? 1 : 0) + (p->dtype == DEDISP_U8 ? 1 : 0);
-}
-
-cudaError_t subband_reserve(dedisp_plan *p, long long nsamp_out, int nbeams) {
-    const long long pitch = (nsamp_out + p->maxshift + 3) & ~3ll;
-    const size_t need = (size_t)nbeams * p->nchans * pitch * sizeof(float);
-    if (need <= p->conv_bytes) return cudaSuccess;
-    if (p->d_conv) cudaFree(p->d_conv);
-    p->d_conv = nullptr;
-    p->conv_bytes = 0;
-    cudaError_t e = cudaMalloc(&p->d_conv, need);
-    if (e == cudaSuccess) p->conv_bytes = need;
-    return e;
+    return (merged ? 1 : (int)p->sb.passes.size()) + (p->dtype == DEDISP_U8 ? 1 : 0);
 }
 
 cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
@@ -634,37 +730,12 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     const int blk_lo = run.blk_lo, blk_hi = run.blk_hi < 0 ? sb.nblk : run.blk_hi;
     const bool whole = run.pass_lo == 0 && pass_hi == npass && blk_lo == 0 && blk_hi == sb.nblk;
     SbArgs A;
-    A.in = (const float *)d_in;
     A.in_stride = in_stride;
     A.in_total = (long long)(p->nchans - 1) * in_stride + nsamp_in;
     A.in_beam = b.in_stride;
     cudaError_t e;
-    if (sb_needs_staging_copy(p, d_in, in_stride, b)) {
-        const long long pitch = (nsamp_in + 3) & ~3ll;
-        const long long obeam = (long long)p->nchans * pitch;
-        e = subband_reserve(p, nsamp_out, b.n);
-        if (e != cudaSuccess) return e;
-        {
-            dim3 grid((unsigned)((nsamp_in + 255) / 256), (unsigned)p->nchans, (unsigned)b.n);
-            switch (p->dtype) {
-                case DEDISP_U8:
-                    dedisp_to_f32_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                    break;
-                case DEDISP_F16:
-                    dedisp_to_f32_kernel<__half><<<grid, 256, 0, st>>>((const __half *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                    break;
-                default:
-                    dedisp_to_f32_kernel<float><<<grid, 256, 0, st>>>((const float *)d_in, in_stride, b.in_stride, p->d_conv, pitch, obeam, nsamp_in);
-                    break;
-            }
-            e = cudaGetLastError();
-            if (e != cudaSuccess) return e;
-        }
-        A.in = p->d_conv;
-        A.in_stride = pitch;
-        A.in_total = obeam;
-        A.in_beam = obeam;
-    }
+    const bool raw = sb_raw_path(p, d_in, in_stride, b);
+    A.in = d_in;
     A.out = d_out;
     A.out_stride = out_stride;
     A.out_beam = b.out_stride;
@@ -680,7 +751,8 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.blk_lo = blk_lo;
     A.blk_hi = blk_hi;
     A.slot_chunks = sb.slot_chunks;
-    A.cb = sb.cb;
+    A.raw_slot_bytes = sb.raw_slot_bytes;
+    A.cb = raw ? sb.cb_raw : sb.cb;
     auto tiles_of = [&](const SubbandPass &ps) -> long long {
         const long long nb = std::min(blk_hi, ps.blk_end) - std::max(blk_lo, ps.blk_begin);
         return nb <= 0 ? 0 : nb * ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * b.n;
@@ -689,7 +761,11 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (tiles <= 0) return cudaSuccess;
         if (tiles >= (1ll << 31)) return cudaErrorInvalidValue;
         const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, p->sm_count));
-        dedisp_subband_kernel<float><<<grid, SB_THREADS, sb.smem, st>>>(A);   // u8 plans too: fp32 sums in place, converted after the last pass
+        // u8 plans too accumulate fp32 sums (exact, checked at plan build) in place; converted after the last pass
+        if (!raw) dedisp_subband_kernel<float, false><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (p->dtype == DEDISP_U8) dedisp_subband_kernel<uint8_t, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
+        else if (p->dtype == DEDISP_F16) dedisp_subband_kernel<__half, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
+        else dedisp_subband_kernel<float, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
         return cudaGetLastError();
     };
     if (whole && sb_merge_passes(p)) {

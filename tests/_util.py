@@ -5,6 +5,8 @@ seeded input (``paper_1111_6399_b200.synth``) to both and compares per element.
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import torch
 
@@ -28,8 +30,22 @@ def make_case(cfg, device="cuda", **kw):
 
 
 def oracle_rows(cfg, x_host: np.ndarray, rows=None, nsamp_out=None):
-    return oracle.dedisperse(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), x_host,
-                             cfg.nsamp_out if nsamp_out is None else nsamp_out, rows=rows)
+    """The oracle on the given DM rows. Many rows of a large plan are split over the host cores: the
+    oracle itself stays single-threaded and unchanged, it is just called on disjoint row subsets from
+    several Python threads (ctypes releases the GIL for the duration of the call)."""
+    nout = cfg.nsamp_out if nsamp_out is None else nsamp_out
+    call = lambda r: oracle.dedisperse(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), x_host, nout, rows=r)
+    rows_arr = np.arange(cfg.ndm, dtype=np.int32) if rows is None else np.asarray(rows, dtype=np.int32)
+    nthreads = min(os.cpu_count() or 1, 32, rows_arr.size)
+    if nthreads < 2 or rows_arr.size * cfg.nchans * nout < 2e9:
+        return call(rows)
+    from concurrent.futures import ThreadPoolExecutor
+    parts = np.array_split(rows_arr, nthreads)
+    with ThreadPoolExecutor(nthreads) as ex:
+        res = list(ex.map(call, parts))
+    if cfg.dtype == "u8":
+        return np.concatenate(res, axis=0)
+    return np.concatenate([r[0] for r in res], axis=0), np.concatenate([r[1] for r in res], axis=0)
 
 
 def assert_matches_oracle(cfg, gpu_out: torch.Tensor, ref, rows=None, what=""):

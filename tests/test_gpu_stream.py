@@ -76,3 +76,39 @@ def test_stream_overlapped_pushes_match_synced():
     for k in range(3):
         assert torch.equal(st.out_view(ptrs[k]), a[k])
     st.close()
+
+
+def test_c5_full_shape_first_chunks_through_the_stream():
+    """configs[4] at its real shape through dedisp_stream_push (SURVEY.md §8(d) "parity coverage at
+    scale"): 32 beams x 1024 channels x 32768-sample chunks, the first 3 chunks, maxshift carried
+    between them; 2 beams x 64 DM rows of every output block against the oracle run on the
+    zero-prefixed concatenated stream."""
+    cfg = CONFIGS["c5"]
+    nchunks, chunk = 3, cfg.nsamp_out
+    plan = P.Plan.from_config(cfg)
+    tab = oracle_table(cfg)
+    maxshift = int(tab.max())
+    assert plan.max_shift == maxshift
+    total = nchunks * chunk
+    beams_checked = (3, 29)
+    host = torch.empty((cfg.nbeams, cfg.nchans, total), dtype=torch.uint8).pin_memory()
+    for b in range(cfg.nbeams):
+        x, _ = synth.make_input(cfg, tab, total, device="cuda", seed=cfg.seed * 1000003 + b * 101,
+                                pulses=[(cfg.ndm - 1, chunk - 5), (cfg.ndm // 3, chunk + 77)])
+        host[b].copy_(x)
+    st = P.Stream(plan, cfg.nbeams, chunk, 2)
+    rows = np.linspace(0, cfg.ndm - 1, 64).round().astype(np.int32)
+    ridx = torch.as_tensor(rows, device="cuda", dtype=torch.long)
+    got = {b: [] for b in beams_checked}
+    for k in range(nchunks):
+        h = host[:, :, k * chunk:(k + 1) * chunk].contiguous().pin_memory()
+        out_ptr, _ = st.push(h)
+        st.sync()
+        view = st.out_view(out_ptr)
+        for b in beams_checked:
+            got[b].append(view[b][ridx].clone())
+    st.close()
+    for b in beams_checked:
+        padded = np.concatenate([np.zeros((cfg.nchans, maxshift), dtype=np.uint8), host[b].numpy()], axis=1)
+        ref = oracle_rows(cfg, np.ascontiguousarray(padded), rows=rows, nsamp_out=total)
+        assert_matches_oracle(cfg, torch.cat(got[b], dim=1), ref, what=f"c5 stream beam {b}")

@@ -152,19 +152,24 @@ def test_tiny_brute_force_per_output():
     rng = np.random.default_rng(5)
     x8 = rng.integers(0, 256, size=(nch, nout + ms), dtype=np.uint8)
     xf = rng.standard_normal((nch, nout + ms)).astype(np.float32)
+    xh = (3.0 * rng.standard_normal((nch, nout + ms))).astype(np.float16)   # oracle_dedisperse_f16 at non-zero shift
     o8 = oracle.dedisperse(nch, fch1, foff, tsamp, dms, x8, nout)
     of, oa = oracle.dedisperse(nch, fch1, foff, tsamp, dms, xf, nout)
+    oh, oha = oracle.dedisperse(nch, fch1, foff, tsamp, dms, xh, nout)
     for t in range(nout):
         for d in range(dms.size):
-            tot8, totf, tota = 0, 0.0, 0.0
+            tot8, totf, tota, toth, totha = 0, 0.0, 0.0, 0.0, 0.0
             for c in reversed(range(nch)):
                 f = fch1 + c * foff
                 s = math.floor(4.148808e3 * dms[d] * (f ** -2 - fch1 ** -2) / tsamp + 0.5)
                 tot8 += int(x8[c, t + s])
                 totf += float(xf[c, t + s])
                 tota += abs(float(xf[c, t + s]))
+                toth += float(xh[c, t + s])          # numpy's own half -> double conversion
+                totha += abs(float(xh[c, t + s]))
             assert o8[d, t] == tot8
             assert abs(of[d, t] - totf) < 1e-12 and abs(oa[d, t] - tota) < 1e-12
+            assert abs(oh[d, t] - toth) < 1e-12 and abs(oha[d, t] - totha) < 1e-12
     assert ms > 20  # the plan actually shifts
 
 
