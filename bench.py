@@ -428,34 +428,69 @@ def run_c5_stream(args, cfg):
     step_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
     value = adds * args.steps / (total_ms * 1e-3) / 1e9
     del out
-    # ---- e2e: the streaming driver, a pool of 3 distinct pinned chunks cycled (generation is outside the timed region)
+    if args.no_e2e:
+        e2e = None
+        del xs
+    else:
+        e2e = _c5_stream_e2e(args, cfg, plan, xs, adds)
+    return _c5_line(args, cfg, plan, hbm_gbs, sm_max_mhz, peak_src, value, total_ms, step_ms, clocks, e2e, adds, nsamp_in)
+
+
+def _c5_stream_e2e(args, cfg, plan, xs, adds):
+    import torch
+    import paper_1111_6399_b200 as P
+    nb, chunk = cfg.nbeams, cfg.nsamp_out
+    # ---- e2e: configs[4]'s stream of 60 consecutive chunks through the streaming driver. The chunks cycle
+    # through a pool of 3 distinct pinned host chunks (generating 60 x 1 GB is outside the method); the
+    # first chunk's block is checked against the oracle outside the timed region.
     pool = [xs[:, :, plan.max_shift - k * 4096: plan.max_shift - k * 4096 + chunk].contiguous().cpu().pin_memory() for k in range(3)]
     del xs
     torch.cuda.empty_cache()
     st = P.Stream(plan, nb, chunk, 3)                     # 3 buffers: block k-1 is still being read while k+1 is enqueued
-    esteps = max(args.steps, 6)
-    h_max = torch.empty((esteps, nb, cfg.ndm), dtype=torch.int32, pin_memory=True)
-    for k in range(2):                                   # warm-up pushes (fills the history)
-        st.push(pool[k % 3])
-    st.sync()
+    nchunks = cfg.nchunks if not args.stream_chunks else args.stream_chunks
+    h_max = torch.empty((nchunks, nb, cfg.ndm), dtype=torch.int32, pin_memory=True)
+    read_done = [torch.cuda.Event() for _ in range(3)]
+
+    def read_block(k, ptr, ev):                           # the consumer: per-(beam, DM) maxima of block k
+        st.wait_event(ev)
+        h_max[k].copy_(st.out_view(ptr).amax(dim=2), non_blocking=True)
+        read_done[k % 3].record()
+        st.release_after(read_done[k % 3])                # the driver may overwrite the block only after this read
+
+    torch.cuda.synchronize()
     t0 = time.perf_counter()
     prev = None
-    for k in range(esteps):
+    for k in range(nchunks):
         ptr, ev = st.push(pool[k % 3])
         if prev is not None:                             # read block k-1's metric while block k computes
-            st.wait_event(prev[1])
-            h_max[k - 1].copy_(st.out_view(prev[0]).amax(dim=2), non_blocking=True)
+            read_block(k - 1, *prev)
         prev = (ptr, ev)
-    st.wait_event(prev[1])
-    h_max[esteps - 1].copy_(st.out_view(prev[0]).amax(dim=2), non_blocking=True)
+    read_block(nchunks - 1, *prev)
     torch.cuda.synchronize()
     et = time.perf_counter() - t0
     st.close()
-    e2e = {"value": adds * esteps / et / 1e9, "unit": UNIT, "h2d_bytes_per_step": pool[0].numel(),
-           "d2h_bytes_per_step": nb * cfg.ndm * 4, "steps": esteps, "ms_per_step": 1e3 * et / esteps,
-           "real_time_factor": chunk * cfg.tsamp / (et / esteps),
-           "api": "dedisp_stream_push (pinned host chunks, 3 device buffers); D2H = per-(beam, DM) maxima of each block"}
-    peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6 / 1e9
+    # check (outside the timed region): block 0 = the first chunk after maxshift zeros; maxima of a few
+    # beams / DM rows from the oracle on exactly that input
+    import numpy as np
+    import oracle
+    rows = np.linspace(0, cfg.ndm - 1, 16).round().astype(np.int32)
+    e2e_ok = True
+    for b in (0, nb - 1):
+        padded = np.concatenate([np.zeros((cfg.nchans, plan.max_shift), dtype=np.uint8), pool[0][b].numpy()], axis=1)
+        ref = oracle.dedisperse(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), np.ascontiguousarray(padded), chunk, rows=rows)
+        e2e_ok = e2e_ok and bool((ref.max(axis=1) == h_max[0, b].numpy()[rows]).all())
+    assert e2e_ok, "streamed block 0 maxima differ from the oracle"
+    e2e = {"value": adds * nchunks / et / 1e9, "unit": UNIT, "h2d_bytes_per_step": pool[0].numel(),
+           "d2h_bytes_per_step": nb * cfg.ndm * 4, "steps": nchunks, "ms_per_step": 1e3 * et / nchunks,
+           "real_time_factor": chunk * cfg.tsamp / (et / nchunks), "e2e_checked": e2e_ok,
+           "api": f"dedisp_stream_push: {nchunks} consecutive chunks (pool of 3 pinned host chunks cycled, 3 device buffers); "
+                  "D2H = per-(beam, DM) maxima of each block, read on a second stream and handed back with dedisp_stream_release_after"}
+    return e2e
+
+
+def _c5_line(args, cfg, plan, hbm_gbs, sm_max_mhz, peak_src, value, total_ms, step_ms, clocks, e2e, adds, nsamp_in):
+    nb, chunk = cfg.nbeams, cfg.nsamp_out
+    peak = add_peak(sm_max_mhz)
     achieved = adds / (step_ms * 1e-3) / 1e9
     kname = {1: "naive", 2: "tiled", 3: "subband"}[plan.kernel]
     bytes_once = nb * (cfg.nchans * nsamp_in + cfg.ndm * chunk * 4)
@@ -525,8 +560,21 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=3.0, help="cpu_baseline: oracle seconds per timed call")
     ap.add_argument("--no-others", action="store_true", help="skip the c2/c4/c5 block of the default line")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stream-chunks", type=int, default=0, help="c5 e2e: chunks pushed (default: the config's 60)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and world_env is None and args.impl == "ours":
+        # plain `python bench.py --gpus N`: start the N ranks ourselves, one process per GPU
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    if world_env is not None and args.impl == "ours" and int(world_env) != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}")
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     from paper_1111_6399_b200 import CONFIGS
     cfg = CONFIGS[args.config]

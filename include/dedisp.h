@@ -174,6 +174,12 @@ int dedisp_stream_push(dedisp_stream *s, const void *h_chunk, void **d_out, void
  * for a done_event returned by dedisp_stream_push, so that work queued on it afterwards may read
  * the block without a host synchronisation. EINVAL on a NULL event. */
 int dedisp_stream_wait_event(void *done_event, void *stream);
+/* dedisp_stream_release_after: a consumer that reads output blocks on its own stream (after
+ * dedisp_stream_wait_event) hands back an event recorded after its last read; every later
+ * dedisp_stream_push computes after that event, so a block is never overwritten (nbuffers pushes later)
+ * while the consumer is still reading it. Without this call the consumer must finish reading block k
+ * before push k + nbuffers is issued (e.g. by dedisp_stream_sync). EINVAL on NULLs. */
+int dedisp_stream_release_after(dedisp_stream *s, void *consumer_event);
 int dedisp_stream_sync(dedisp_stream *s);
 int dedisp_stream_destroy(dedisp_stream *s);
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
     "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_error_string",
-    "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_sync",
+    "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_release_after", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
 
@@ -77,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_stream_create.argtypes = [ctypes.POINTER(vp), vp, c_int, c_ll, c_int]
         L.dedisp_stream_push.argtypes = [vp, vp, ctypes.POINTER(vp), ctypes.POINTER(vp)]
         L.dedisp_stream_wait_event.argtypes = [vp, vp]
+        L.dedisp_stream_release_after.argtypes = [vp, vp]
         L.dedisp_stream_sync.argtypes = [vp]
         L.dedisp_stream_destroy.argtypes = [vp]
         _lib = L
@@ -258,6 +259,11 @@ class Stream:
     def wait_event(self, event_ptr: int, stream=None) -> None:
         """``dedisp_stream_wait_event``: ``stream`` (default: torch's current) waits for a block's done event."""
         self.plan._check(lib().dedisp_stream_wait_event(event_ptr, _stream_ptr(stream)), "dedisp_stream_wait_event")
+
+    def release_after(self, event: "torch.cuda.Event") -> None:
+        """Later pushes compute after `event` (recorded by the consumer after its last read of a block)."""
+        self.plan._check(lib().dedisp_stream_release_after(self._h, ctypes.c_void_p(event.cuda_event)),
+                         "dedisp_stream_release_after")
 
     def sync(self) -> None:
         self.plan._check(lib().dedisp_stream_sync(self._h), "dedisp_stream_sync")

@@ -132,6 +132,14 @@ int dedisp_stream_wait_event(void *done_event, void *stream) {
     return cudaStreamWaitEvent((cudaStream_t)stream, (cudaEvent_t)done_event, 0) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
 }
 
+int dedisp_stream_release_after(dedisp_stream *s, void *consumer_event) {
+    if (!s || !consumer_event) return DEDISP_EINVAL;
+    // every later launch on the compute stream (i.e. every later overwrite of an output block) is
+    // ordered after the consumer's event
+    const cudaError_t e = cudaStreamWaitEvent(s->comp_st, (cudaEvent_t)consumer_event, 0);
+    return e == cudaSuccess ? DEDISP_OK : stream_fail(s, e, "dedisp_stream_release_after");
+}
+
 int dedisp_stream_sync(dedisp_stream *s) {
     if (!s) return DEDISP_EINVAL;
     cudaError_t e = cudaStreamSynchronize(s->copy_st);

@@ -110,6 +110,41 @@ def test_strided_and_batched(kernel):
     assert bool((outs[:, cfg.ndm:] == -7).all()) and bool((outs[:, :, cfg.nsamp_out:] == -7).all())
 
 
+def test_concurrent_executes_on_two_streams():
+    """§8(b) ownership: dedisp_execute allocates nothing and leaves the plan read-only for every dtype, so
+    two calls on ONE plan may run concurrently on different streams (u8 input: the raw path converts
+    inside the kernel, there is no shared scratch)."""
+    cfg = SMALL["c2s"]
+    plan = _plan_with(cfg, P.KERNEL_SUBBAND)
+    xs = [make_case(cfg, seed=700 + i)[0] for i in range(2)]
+    outs = [plan.alloc_out(cfg.nsamp_out) for _ in range(2)]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for i in range(2):
+            plan.execute(xs[i], cfg.nsamp_out, outs[i], stream=streams[i])
+    torch.cuda.synchronize()
+    for i in range(2):
+        assert_matches_oracle(cfg, outs[i], oracle_rows(cfg, xs[i].cpu().numpy()), what=f"stream {i}")
+
+
+def test_unaligned_fp32_rows_take_the_raw_path():
+    """fp32 rows whose base / pitch are not 16-byte aligned: SUBBAND realigns them in its raw path (no
+    silent drop to the NAIVE kernel)."""
+    cfg = SMALL["c3s"]
+    plan = _plan_with(cfg, P.KERNEL_SUBBAND)
+    x, tab, _ = make_case(cfg)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    pitch = nsamp_in + 3 - (nsamp_in % 2)                       # odd pitch: rows start at every 4-byte phase
+    buf = torch.zeros(cfg.nchans * pitch + 5, dtype=torch.float32, device="cuda")
+    view = buf[1:1 + cfg.nchans * pitch].view(cfg.nchans, pitch)[:, :nsamp_in]    # base off by 4 bytes
+    view.copy_(x)
+    out = plan.execute(view, cfg.nsamp_out)
+    torch.cuda.synchronize()
+    assert plan.kernel == P.KERNEL_SUBBAND
+    assert_matches_oracle(cfg, out, oracle_rows(cfg, x.cpu().numpy()), what="unaligned fp32 rows")
+
+
 def test_errors():
     cfg = CONFIGS["c1"]
     plan = P.Plan.from_config(cfg)
