@@ -147,6 +147,11 @@ long long dedisp_plan_verify_records(const dedisp_plan *plan);
 /* Number of kernel launches one dedisp_execute issues for this plan (for bench.py's gpu_launches). */
 int dedisp_plan_launches_per_execute(const dedisp_plan *plan);
 
+/* Launch geometry of the SUBBAND kernel for this plan, for reports: h_out[8] = {channels per pipeline
+ * stage (aligned fp32 rows), the same for the raw path (u8 / f16 / unaligned rows), bytes per staged
+ * channel window, dynamic shared memory of the two paths, DM blocks, DM ranges, passes}. Zeros if the
+ * plan does not admit SUBBAND. */
+int dedisp_plan_get_geometry(const dedisp_plan *plan, int *h_out);
 /* Number of DM slabs the last dedisp_execute_host call on this plan ran its final pass in (0: the
  * call did not take the slab-overlap path). For the tests that must know which path they exercised. */
 int dedisp_plan_last_host_slabs(const dedisp_plan *plan);

@@ -30,7 +30,7 @@ SYMBOLS = (
     "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
-    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_error_string",
+    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_error_string",
     "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_release_after", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
@@ -68,6 +68,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_plan_set_kernel.argtypes = [vp, c_int]
         L.dedisp_plan_set_pass_merge.argtypes = [vp, c_int]
         L.dedisp_plan_get_subbands.argtypes = [vp, ip]
+        L.dedisp_plan_get_geometry.argtypes = [vp, ip]
         L.dedisp_plan_verify_records.argtypes = [vp]
         L.dedisp_plan_verify_records.restype = c_ll
         L.dedisp_error_string.argtypes = [c_int]
@@ -164,6 +165,12 @@ class Plan:
         self._check(lib().dedisp_plan_get_subbands(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int))),
                     "dedisp_plan_get_subbands")
         return out
+
+    def geometry(self) -> dict:
+        v = np.zeros(8, dtype=np.int32)
+        self._check(lib().dedisp_plan_get_geometry(self._h, v.ctypes.data_as(ctypes.POINTER(ctypes.c_int))), "dedisp_plan_get_geometry")
+        keys = ("cb", "cb_raw", "slot_bytes", "smem", "smem_raw", "nblk", "nranges", "npasses")
+        return dict(zip(keys, (int(x) for x in v)))
 
     def verify_records(self) -> int:
         return int(lib().dedisp_plan_verify_records(self._h))

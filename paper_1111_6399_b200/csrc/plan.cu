@@ -299,6 +299,15 @@ long long dedisp_plan_verify_records(const dedisp_plan *p) {
     return subband_verify_records(p);
 }
 
+int dedisp_plan_get_geometry(const dedisp_plan *p, int *h_out) {
+    if (!p || !h_out) return DEDISP_EINVAL;
+    const SubbandGeom &sb = p->sb;
+    const int v[8] = {sb.ok ? sb.cb : 0, sb.ok ? sb.cb_raw : 0, sb.slot_chunks * 16, (int)sb.smem, (int)sb.smem_raw,
+                      sb.nblk, sb.nranges, (int)sb.passes.size()};
+    std::memcpy(h_out, v, sizeof v);
+    return DEDISP_OK;
+}
+
 int dedisp_plan_last_host_slabs(const dedisp_plan *p) { return p ? p->host_slabs : -1; }
 
 int dedisp_plan_launches_per_execute(const dedisp_plan *p) {

@@ -51,6 +51,11 @@ constexpr int SB_CB = SB_CB_CFG;      // smallest number of channels per pipelin
 #define SB_STAGES_CFG 2
 #endif
 constexpr int SB_STAGES = SB_STAGES_CFG;
+#ifndef SB_CB_MAX_CFG
+#define SB_CB_MAX_CFG 16
+#endif
+constexpr int SB_CB_MAX = SB_CB_MAX_CFG;  // channels per stage are chosen at plan build (as many as fit, at most this)
+constexpr int SB_EP_WORDS = SB_T + 8;     // epilogue transpose buffer of one warp: one row of the tile, shifted by up to 3 words
 // staged 16-byte chunks per channel the slot can hold, a multiple of 32
 constexpr int SB_NCH_MAX = ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 * 32;
 

@@ -120,6 +120,20 @@ int pick_ref(const dedisp_plan *p, int cb, int ce) {
 
 }  // namespace
 
+// raw path: bytes per raw channel slot (window bytes + up to 15 lead bytes, rounded up to 16, + one
+// spare chunk the realigning loads may touch)
+static int sb_raw_slot_bytes(int slot_chunks, int esize) { return ((slot_chunks * 4 * esize + 15 + 15) & ~15) + 16; }
+
+// dynamic shared memory of the SUBBAND kernel for `cb` channels per stage (esize > 0: raw path)
+static size_t sb_smem_bytes(int cb, int slot_chunks, int esize) {
+    size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES + 16;
+    b = (b + 15) / 16 * 16;
+    b += (size_t)SB_WARPS * SB_EP_WORDS * sizeof(float);
+    if (esize > 0) b += (size_t)cb * sb_raw_slot_bytes(slot_chunks, esize);
+    return b;
+}
+
+
 void subband_build(dedisp_plan *p) {
     p->sb = SubbandGeom();
     SubbandGeom &sb = p->sb;
@@ -149,9 +163,10 @@ void subband_build(dedisp_plan *p) {
     sb.nranges = (int)range_begin.size() - 1;
     for (int r = 0; r < sb.nranges; ++r) {
         const int b0 = range_begin[r], b1 = range_begin[r + 1];
-        // greedy: extend each sub-band as far as the geometry admits (exponential then binary search)
+        // greedy from the top of the band: extend each sub-band as far as the geometry admits (exponential
+        // then binary search)
+        std::vector<SubbandPass> cut;
         int cb = 0;
-        bool first = true;
         while (cb < nchans) {
             auto ok = [&](int ce) { return pass_geometry(p, cb, ce, pick_ref(p, cb, ce), false, b0, b1); };
             if (!ok(cb + 1)) { sb = SubbandGeom(); return; }  // a single channel against itself always has r = 0; defensive
@@ -172,14 +187,27 @@ void subband_build(dedisp_plan *p) {
             SubbandPass ps;
             ps.c_begin = cb;
             ps.c_end = good;
-            ps.c_ref = pick_ref(p, cb, good);
             ps.blk_begin = b0;
             ps.blk_end = b1;
-            ps.first = first;
-            first = false;
-            sb.passes.push_back(ps);
+            cut.push_back(ps);
             cb = good;
-            if (sb.passes.size() > 2048) { sb = SubbandGeom(); return; }  // hopelessly coarse plan: use TILED
+            if (cut.size() > 2048) { sb = SubbandGeom(); return; }  // hopelessly coarse plan: use TILED
+        }
+        // the greedy cut leaves whatever remains to the last sub-band; a pass of a few channels still costs a
+        // whole sweep over out (c3: 8 channels, 1.0 ms), so share the channels of the last two evenly
+        if (cut.size() >= 2) {
+            SubbandPass &u = cut[cut.size() - 2], &v = cut.back();
+            const int mid = (u.c_begin + v.c_end) / 2;
+            if (v.c_end - v.c_begin < (u.c_end - u.c_begin) / 2 && mid > u.c_begin && mid <= u.c_end &&
+                pass_geometry(p, mid, v.c_end, pick_ref(p, mid, v.c_end), false, b0, b1)) {
+                u.c_end = mid;
+                v.c_begin = mid;
+            }
+        }
+        for (size_t i = 0; i < cut.size(); ++i) {
+            cut[i].c_ref = pick_ref(p, cut[i].c_begin, cut[i].c_end);
+            cut[i].first = i == 0;
+            sb.passes.push_back(cut[i]);
         }
     }
     sb.records.assign((size_t)nchans * gslots, 0);
@@ -194,6 +222,18 @@ void subband_build(dedisp_plan *p) {
     }
     // the kernel's dynamic shared memory (ring + records + transpose buffers) must fit the 227 KB a CTA may opt into
     if (!subband_smem_fits(p)) { sb = SubbandGeom(); return; }
+    // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
+    sb.slot_chunks = sb.max_nch + 1;
+    const int esize = dtype_esize(p->dtype);
+    sb.raw_slot_bytes = sb_raw_slot_bytes(sb.slot_chunks, esize);
+    auto pick = [&](int es, int &cb_out, size_t &smem_out) {
+        cb_out = SB_CB;
+        for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
+            if (sb_smem_bytes(cb, sb.slot_chunks, es) <= 227u * 1024u) { cb_out = cb; break; }
+        smem_out = sb_smem_bytes(cb_out, sb.slot_chunks, es);
+    };
+    pick(0, sb.cb, sb.smem);
+    pick(esize, sb.cb_raw, sb.smem_raw);
     sb.ok = true;
 }
 
@@ -254,10 +294,6 @@ template <bool RAW> struct SbRegs { static constexpr int consumer = RAW ? 152 : 
 static_assert(SB_CONSUMERS * SbRegs<false>::consumer + 128 * SbRegs<false>::producer <= 65536, "register file");
 static_assert(SB_CONSUMERS * SbRegs<true>::consumer + 128 * SbRegs<true>::producer <= 65536, "register file");
 static_assert(SB_STAGES >= 2, "ring depth");
-#ifndef SB_CB_MAX_CFG
-#define SB_CB_MAX_CFG 16
-#endif
-constexpr int SB_CB_MAX = SB_CB_MAX_CFG;             // channels per stage are chosen at launch (as many as fit)
 static_assert(SB_CB_MAX <= 32 && SB_CB <= SB_CB_MAX, "one producer lane per staged channel");
 static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 
@@ -321,7 +357,6 @@ struct SbArgs {
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
 };
 
-constexpr int SB_EP_PITCH = SB_K + 4;  // epilogue transpose: words per lane, an odd number of 8-byte pairs
 typedef unsigned long long sb_u64;     // one aligned register pair = two fp32 accumulators (FADD2 operand)
 
 // The CTA's next non-empty tile. Tiles of a pass are numbered beam-major, then u-tile, then DM block
@@ -402,7 +437,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
     const unsigned bar_raw_full = bar_empty + 8u * SB_STAGES, bar_raw_empty = bar_raw_full + 8u;
     const unsigned ep_off = (bar_raw_empty + 8u - sdata_base + 15u) & ~15u;
-    const unsigned raw_base = sdata_base + ep_off + SB_WARPS * 32 * SB_EP_PITCH * 4;
+    const unsigned raw_base = sdata_base + ep_off + SB_WARPS * SB_EP_WORDS * 4;
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, RAW ? 4 : 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
@@ -536,7 +571,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     // ---------------- consumer warps
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SbRegs<RAW>::consumer));
     const unsigned sdata_u32 = sdata_base + 4u * SB_K * lane;
-    float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * (32 * SB_EP_PITCH);
+    float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * SB_EP_WORDS;
     while (sb_next_tile(A, t)) {
         sb_u64 acc[SB_D][SB_K / 2];
 #pragma unroll
@@ -558,60 +593,63 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 
         // Epilogue: a lane holds SB_K consecutive samples of each row, so direct stores would touch 32
         // sectors per instruction. Each warp transposes row by row through its own buffer and writes /
-        // adds out[d][t] with lanes on consecutive 16-byte groups; no other warp is involved.
-        OutT *out = reinterpret_cast<OutT *>(A.out) + (size_t)t.beam * A.out_beam;
+        // adds out[d][t] with lanes on consecutive 16-byte groups; no other warp is involved. The row is
+        // parked SHIFTED by sh = skew(d) mod 4 words, so that the groups that are 16-byte aligned in out
+        // are 16-byte aligned in the buffer too: one LDS.128 + one vector store / reduction per group.
+        float *out = reinterpret_cast<float *>(A.out) + (size_t)t.beam * A.out_beam;
         const int d0 = t.blk * SB_ROWS + warp * SB_D;
         const int first = A.first;
+        const unsigned ep_u32 = (unsigned)__cvta_generic_to_shared(ep);
 #pragma unroll
         for (int j = 0; j < SB_D; ++j) {
             const int d = d0 + j;
             if (d >= A.ndm) break;
+            const long long t0 = t.U0 - (long long)__ldg(t.skew + d);      // t of the tile's sample 0
+            float *orow = out + (size_t)d * A.out_stride;
+            const int sh = A.out_vec4 ? (int)(t0 & 3) : 0;                 // word 4g of the buffer <-> t = t0 - sh + 4g
             __syncwarp();
+            const unsigned wbase = ep_u32 + 4u * (unsigned)(SB_K * lane + sh);
+            if (!(sh & 1)) {
 #pragma unroll
-            for (int k2 = 0; k2 < SB_K / 2; ++k2)
-                *reinterpret_cast<sb_u64 *>(ep + lane * SB_EP_PITCH + 2 * k2) = acc[j][k2];
-            __syncwarp();
-            const long long t0 = t.U0 - (long long)__ldg(t.skew + d);
-            OutT *orow = out + (size_t)d * A.out_stride;
-            auto E = [&](int sidx) { return ep[(sidx / SB_K) * SB_EP_PITCH + (sidx % SB_K)]; };
-            auto put = [&](int sidx) {                           // one sample, bounds-checked
-                const long long tt = t0 + sidx;
-                if (tt >= 0 && tt < A.nsamp_out) {
-                    if constexpr (sizeof(OutT) == 4 && !std::is_floating_point<OutT>::value) {
-                        const int vi = __float2int_rn(E(sidx));
-                        orow[tt] = first ? vi : orow[tt] + vi;
-                    } else {
-                        if (first) orow[tt] = E(sidx);
-                        else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + tt), "f"(E(sidx)) : "memory");
-                    }
-                }
-            };
-            if constexpr (std::is_floating_point<OutT>::value) {
-                if (A.out_vec4) {
-                    // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
-                    // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
-                    const int m = (int)((-t0) & 3);              // samples before the first aligned t
-                    const int nv = (SB_T - m) / 4;
-#pragma unroll 1
-                    for (int v = lane; v < nv; v += 32) {
-                        const int sidx = m + 4 * v;
-                        const long long tt = t0 + sidx;
-                        if (tt >= 0 && tt + 3 < A.nsamp_out) {
-                            const float x0 = E(sidx), x1 = E(sidx + 1), x2 = E(sidx + 2), x3 = E(sidx + 3);
-                            if (first) *reinterpret_cast<float4 *>(orow + tt) = make_float4(x0, x1, x2, x3);
-                            else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
-                                              ::"l"(orow + tt), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
-                        } else {
-                            put(sidx); put(sidx + 1); put(sidx + 2); put(sidx + 3);
-                        }
-                    }
-                    if (lane < m) put(lane);                                             // head
-                    if (lane < SB_T - (m + 4 * nv)) put(m + 4 * nv + lane);              // tail
-                    continue;
+                for (int k2 = 0; k2 < SB_K / 2; ++k2)
+                    asm volatile("st.shared.b64 [%0], %1;\n" ::"r"(wbase + 8u * k2), "l"(acc[j][k2]) : "memory");
+            } else {
+#pragma unroll
+                for (int k2 = 0; k2 < SB_K / 2; ++k2) {
+                    asm volatile("st.shared.b32 [%0], %1;\n" ::"r"(wbase + 8u * k2), "r"((unsigned)acc[j][k2]) : "memory");
+                    asm volatile("st.shared.b32 [%0], %1;\n" ::"r"(wbase + 8u * k2 + 4u), "r"((unsigned)(acc[j][k2] >> 32)) : "memory");
                 }
             }
+            __syncwarp();
+            auto put = [&](int w) {                              // one buffer word, bounds-checked
+                const int sidx = w - sh;
+                const long long tt = t0 + sidx;
+                if (sidx >= 0 && sidx < SB_T && tt >= 0 && tt < A.nsamp_out) {
+                    if (first) orow[tt] = ep[w];
+                    else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + tt), "f"(ep[w]) : "memory");
+                }
+            };
+            if (A.out_vec4) {
+                // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
+                // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
 #pragma unroll 1
-            for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
+                for (int g = lane; g < (SB_T + 3 + 3) / 4; g += 32) {
+                    const int sidx = 4 * g - sh;
+                    const long long tt = t0 + sidx;
+                    if (sidx >= 0 && sidx + 3 < SB_T && tt >= 0 && tt + 3 < A.nsamp_out) {
+                        float4 v;
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(ep_u32 + 16u * g));
+                        if (first) *reinterpret_cast<float4 *>(orow + tt) = v;
+                        else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
+                                          ::"l"(orow + tt), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+                    } else {
+                        put(4 * g); put(4 * g + 1); put(4 * g + 2); put(4 * g + 3);
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
+            }
         }
     }
 }
@@ -624,19 +662,6 @@ __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__r
     if (i >= nsamp_out) return;
     int *pv = out + (size_t)blockIdx.z * out_beam + (size_t)(d0 + blockIdx.y) * out_stride + i;
     *pv = __float2int_rn(__int_as_float(*pv));
-}
-
-// raw path: bytes per raw channel slot (window bytes + up to 15 lead bytes, rounded up to 16, + one
-// spare chunk the realigning loads may touch)
-int sb_raw_slot_bytes(int slot_chunks, int esize) { return ((slot_chunks * 4 * esize + 15 + 15) & ~15) + 16; }
-
-// dynamic shared memory of the SUBBAND kernel for `cb` channels per stage (esize > 0: raw path)
-size_t sb_smem_bytes(int cb, int slot_chunks, int esize) {
-    size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES + 16;
-    b = (b + 15) / 16 * 16;
-    b += (size_t)SB_WARPS * 32 * SB_EP_PITCH * sizeof(float);
-    if (esize > 0) b += (size_t)cb * sb_raw_slot_bytes(slot_chunks, esize);
-    return b;
 }
 
 }  // namespace
@@ -661,18 +686,6 @@ cudaError_t subband_upload(dedisp_plan *p) {
     if (e == cudaSuccess) e = cudaMalloc(&sb.d_skew, sb.skew.size() * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_skew, sb.skew.data(), sb.skew.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
-    // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
-    sb.slot_chunks = sb.max_nch + 1;
-    const int esize = dtype_esize(p->dtype);
-    sb.raw_slot_bytes = sb_raw_slot_bytes(sb.slot_chunks, esize);
-    auto pick = [&](int es, int &cb_out, size_t &smem_out) {
-        cb_out = SB_CB;
-        for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
-            if (sb_smem_bytes(cb, sb.slot_chunks, es) <= 227u * 1024u) { cb_out = cb; break; }
-        smem_out = sb_smem_bytes(cb_out, sb.slot_chunks, es);
-    };
-    pick(0, sb.cb, sb.smem);
-    pick(esize, sb.cb_raw, sb.smem_raw);
     switch (p->dtype) {
         case DEDISP_U8: return cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
         case DEDISP_F16: return cudaFuncSetAttribute(dedisp_subband_kernel<__half, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
