@@ -526,6 +526,11 @@ def run_paper_sweep(args):
     for nchans, max_dm in points:
         cfg = paper_sweep(nchans, max_dm)
         plan = P.Plan.from_config(cfg)
+        if args.kernel:
+            try:
+                plan.set_kernel({"naive": 1, "tiled": 2, "subband": 3}[args.kernel])
+            except P.DedispError:
+                continue
         x, _ = synth.make_input(cfg, plan.shifts(), cfg.nsamp_out + plan.max_shift, device="cuda")
         out = plan.alloc_out(cfg.nsamp_out)
         for _ in range(args.warmup):

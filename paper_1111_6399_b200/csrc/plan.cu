@@ -16,7 +16,14 @@ int fail_cuda(dedisp_plan *p, cudaError_t e, const char *what) {
 
 int resolve_kernel(const dedisp_plan *p) {
     int k = p->kernel;
-    if (k == DEDISP_KERNEL_AUTO) k = p->sb.ok ? DEDISP_KERNEL_SUBBAND : p->tiled.ok ? DEDISP_KERNEL_TILED : DEDISP_KERNEL_NAIVE;
+    if (k == DEDISP_KERNEL_AUTO) {
+        // SUBBAND pays a tile prologue + epilogue per pass worth about 20 channels of its inner loop, TILED
+        // runs at a flat ~13 % of the add peak: plans cut into passes shorter than that (the paper-regime
+        // sweeps at 250 / 500 channels: 3 and 13 channels per pass) are faster on TILED (profiles/r2_paper_sweep.md)
+        const bool short_passes = p->sb.ok && p->tiled.ok &&
+                                  (long long)p->nchans * p->sb.nranges < 20ll * (long long)p->sb.passes.size();
+        k = p->sb.ok && !short_passes ? DEDISP_KERNEL_SUBBAND : p->tiled.ok ? DEDISP_KERNEL_TILED : DEDISP_KERNEL_NAIVE;
+    }
     return k;
 }
 

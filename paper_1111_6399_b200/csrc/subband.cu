@@ -325,10 +325,15 @@ __device__ __forceinline__ void sb_mbar_arrive(unsigned bar) {
 __device__ __forceinline__ void sb_mbar_arrive_cp_async(unsigned bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
 }
+#ifndef SB_SLEEP_NS
+#define SB_SLEEP_NS 256
+#endif
+#define SB_STR2(x) #x
+#define SB_STR(x) SB_STR2(x)
 // producer side: the slot is usually still being read, so sleep instead of spinning on the issue slots
 // of the consumer warps that share this scheduler
 __device__ __forceinline__ void sb_mbar_wait_sleep(unsigned bar, unsigned parity) {
-    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1, %2;\n@p bra.uni DONE_%=;\nnanosleep.u32 256;\nbra.uni WAIT_%=;\nDONE_%=:\n}\n"
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1, %2;\n@p bra.uni DONE_%=;\nnanosleep.u32 " SB_STR(SB_SLEEP_NS) ";\nbra.uni WAIT_%=;\nDONE_%=:\n}\n"
                  ::"r"(bar), "r"(parity), "r"(100000u) : "memory");
 }
 __device__ __forceinline__ void sb_mbar_wait(unsigned bar, unsigned parity) {

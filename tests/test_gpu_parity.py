@@ -145,6 +145,38 @@ def test_unaligned_fp32_rows_take_the_raw_path():
     assert_matches_oracle(cfg, out, oracle_rows(cfg, x.cpu().numpy()), what="unaligned fp32 rows")
 
 
+@pytest.mark.parametrize("kernel", KERNELS, ids=[KNAME[k] for k in KERNELS])
+@pytest.mark.parametrize("name,lead", [("c3s", 0), ("c3s", 3), ("c2s", 0), ("c2s", 5), ("c4s", 1)])
+def test_guard_bands_are_never_summed(name, lead, kernel):
+    """compute-sanitizer is closed on this pool, so out-of-bounds reads are hunted with poison instead:
+    the input rows sit in a larger buffer whose every other element (in front of the first row, in the
+    pitch padding between rows, behind the last row) holds a value that would wreck any sum it entered
+    (NaN for fp, 255 for u8 with the oracle run on the clean rows); `lead` elements in front make the base
+    unaligned. The output must still equal the oracle's, and the canaries around out must survive."""
+    cfg = SMALL[name]
+    plan = _plan_with(cfg, kernel)
+    x, tab, _ = make_case(cfg)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    per16 = 16 // x.element_size()
+    pitch = (nsamp_in + 2 * per16 + per16 - 1) // per16 * per16 + (1 if lead else 0) * 0
+    poison = 255 if cfg.dtype == "u8" else float("nan")
+    buf = torch.full((64 + lead + cfg.nchans * pitch + 64,), poison, dtype=x.dtype, device="cuda")
+    view = buf[64 + lead: 64 + lead + cfg.nchans * pitch].view(cfg.nchans, pitch)[:, :nsamp_in]
+    view.copy_(x)
+    obuf = torch.full((cfg.ndm + 2, cfg.nsamp_out + 8), -7, dtype=torch.int32 if cfg.dtype == "u8" else torch.float32, device="cuda")
+    out = obuf[1:cfg.ndm + 1, 4:4 + cfg.nsamp_out]
+    if kernel == P.KERNEL_TILED and (view.data_ptr() & 15):
+        with pytest.raises(P.DedispError) as ei:      # TILED, when forced, wants a 16-byte-aligned base (dedisp.h)
+            plan.execute(view, cfg.nsamp_out, out)
+        assert ei.value.code == 1
+        return
+    plan.execute(view, cfg.nsamp_out, out)
+    torch.cuda.synchronize()
+    assert_matches_oracle(cfg, out, oracle_rows(cfg, x.cpu().numpy()), what=f"{name}/{KNAME[kernel]} lead {lead}")
+    assert bool((obuf[0] == -7).all()) and bool((obuf[-1] == -7).all())
+    assert bool((obuf[:, :4] == -7).all()) and bool((obuf[:, 4 + cfg.nsamp_out:] == -7).all())
+
+
 def test_errors():
     cfg = CONFIGS["c1"]
     plan = P.Plan.from_config(cfg)
@@ -252,6 +284,10 @@ def test_execute_host_matches_oracle(name):
         tab = oracle_table(cfg)
         cfg = shrink(cfg, nsamp_out=cfg.nsamp_out + (-(cfg.nsamp_out + int(tab.max())) % 4))
     plan = P.Plan.from_config(cfg)
+    try:
+        plan.set_kernel(P.KERNEL_SUBBAND)     # the overlapped copies belong to SUBBAND (AUTO may prefer TILED for coarse plans)
+    except P.DedispError:
+        pass
     for seed in (11, 12):
         x, tab, _ = make_case(cfg, device="cpu", seed=seed)
         h_in = x.pin_memory()
@@ -269,7 +305,8 @@ def test_execute_host_slab_branch_matches_oracle():
     tab = oracle_table(cfg)
     cfg = shrink(cfg, nsamp_out=cfg.nsamp_out + (-(cfg.nsamp_out + int(tab.max())) % 4))
     plan = P.Plan.from_config(cfg)
-    assert plan.kernel == P.KERNEL_SUBBAND and plan.num_subbands() > 1 and (cfg.nsamp_out + plan.max_shift) % 4 == 0
+    plan.set_kernel(P.KERNEL_SUBBAND)     # (AUTO would pick TILED for a plan this coarse: passes of a few channels)
+    assert plan.num_subbands() > 1 and (cfg.nsamp_out + plan.max_shift) % 4 == 0
     for seed in (21, 22):
         x, _, _ = make_case(cfg, device="cpu", seed=seed)
         out = plan.execute_host(x.pin_memory(), cfg.nsamp_out)
@@ -284,6 +321,7 @@ def test_execute_host_with_merged_passes():
     tab = oracle_table(cfg)
     cfg = shrink(cfg, nsamp_out=cfg.nsamp_out + (-(cfg.nsamp_out + int(tab.max())) % 4))
     plan = P.Plan.from_config(cfg)
+    plan.set_kernel(P.KERNEL_SUBBAND)
     plan.set_pass_merge(True)
     x, _, _ = make_case(cfg, device="cpu", seed=31)
     out = plan.execute_host(x.pin_memory(), cfg.nsamp_out)
