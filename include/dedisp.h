@@ -41,7 +41,8 @@ enum dedisp_status {
     DEDISP_EUNSUPPORTED = 4  /* device is not sm_100, or maxshift >= 2^31, or plan is host-only */
 };
 
-/* Kernel selection (dedisp_plan_set_kernel). AUTO picks SUBBAND when the plan admits it, else TILED.
+/* Kernel selection (dedisp_plan_set_kernel). AUTO picks SUBBAND when the plan admits it and its passes
+ * are not too short (about 20 channels per pass on average), else TILED, else NAIVE.
  * NAIVE is the one-thread-per-(d,t) cross-check kernel used by the parity tests' chain of trust. */
 enum dedisp_kernel {
     DEDISP_KERNEL_AUTO = 0,
@@ -81,17 +82,19 @@ int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1_mhz, doubl
  *          nsamp_out + dedisp_plan_max_shift(plan)); channel 0 = fch1 (highest frequency).
  *   d_out: [ndm][nsamp_out], row stride nsamp_out; int32 for DEDISP_U8 input (exact), float32 for
  *          DEDISP_F16 / DEDISP_F32 input (fp32 accumulation; summation order unspecified).
- * May be called repeatedly. With DEDISP_F32 input whose base and row pitch are 16-byte aligned the
- * call allocates nothing and the plan is read-only, so concurrent calls on different streams are
- * allowed. With DEDISP_U8 / DEDISP_F16 input (or unaligned rows) the SUBBAND kernel first converts
- * the input into a plan-owned fp32 scratch copy (grown on demand with cudaMalloc, freed at destroy):
- * calls on one plan must then be ordered on one stream. EINVAL: NULLs, nsamp_out < 1. */
+ * May be called repeatedly. The call allocates nothing, does not synchronise, and leaves the plan
+ * read-only for every input dtype, so calls on one plan may run concurrently on different streams.
+ * (u8 / f16 input and fp32 rows that are not 16-byte aligned are converted / realigned inside the
+ * SUBBAND kernel's staging step; there is no scratch copy of the input.) EINVAL: NULLs, nsamp_out < 1. */
 int dedisp_execute(dedisp_plan *plan, const void *d_in, long long nsamp_out, void *d_out,
                    void *stream);
 
 /* Same with explicit row strides in ELEMENTS (in_stride >= nsamp_out + maxshift, out_stride >=
- * nsamp_out), else EINVAL. A 16-byte-aligned d_in and in_stride*elemsize let the staging use
- * 16-byte transactions; any stride is correct. */
+ * nsamp_out), else EINVAL. Any base address and any stride are correct; a 16-byte-aligned d_in and
+ * in_stride*elemsize let fp32 input take the direct TMA path, a 16-byte-aligned d_out and
+ * out_stride*4 let the epilogue use vector stores / reductions. The TILED kernel, when forced with
+ * dedisp_plan_set_kernel, requires a 16-byte-aligned d_in (EINVAL otherwise); AUTO never fails on
+ * alignment. */
 int dedisp_execute_strided(dedisp_plan *plan, const void *d_in, long long in_stride_elems,
                            long long nsamp_out, void *d_out, long long out_stride_elems,
                            void *stream);
