@@ -87,7 +87,8 @@ struct SbRun {
 
 struct SubbandGeom {
     bool ok = false;
-    std::vector<SubbandPass> passes;
+    std::vector<SubbandPass> passes;  // launch order: the k-th sub-band of every DM range, k = 0, 1, ...
+    std::vector<int> launch_begin;    // [nlaunch + 1]: ordered launch g runs passes [launch_begin[g], launch_begin[g + 1])
     int ngroups = 0, nblk = 0;
     int nranges = 0;                  // DM-block ranges, each with its own sub-band partition (1 for uniform DM plans)
     // [nblk][nchans][SB_WARPS] per (block, channel, group): low word = joint pattern ids, 8 bits per dispatch group (group 0 lowest):

@@ -161,6 +161,7 @@ void subband_build(dedisp_plan *p) {
         range_begin.push_back(sb.nblk);
     }
     sb.nranges = (int)range_begin.size() - 1;
+    std::vector<std::vector<SubbandPass>> cuts(sb.nranges);
     for (int r = 0; r < sb.nranges; ++r) {
         const int b0 = range_begin[r], b1 = range_begin[r + 1];
         // greedy from the top of the band: extend each sub-band as far as the geometry admits (exponential
@@ -207,9 +208,24 @@ void subband_build(dedisp_plan *p) {
         for (size_t i = 0; i < cut.size(); ++i) {
             cut[i].c_ref = pick_ref(p, cut[i].c_begin, cut[i].c_end);
             cut[i].first = i == 0;
-            sb.passes.push_back(cut[i]);
         }
+        cuts[r] = cut;
     }
+    // launch k runs the k-th sub-band of EVERY DM range (they touch disjoint rows of out, so their order
+    // within a launch is free): a plan with three ranges (c4) needs a third of the launches, each with
+    // three times the tiles to balance over the SMs
+    sb.launch_begin.clear();
+    for (size_t k = 0;; ++k) {
+        bool any = false;
+        for (int r = 0; r < sb.nranges; ++r)
+            if (k < cuts[r].size()) {
+                if (!any) sb.launch_begin.push_back((int)sb.passes.size());
+                any = true;
+                sb.passes.push_back(cuts[r][k]);
+            }
+        if (!any) break;
+    }
+    sb.launch_begin.push_back((int)sb.passes.size());
     sb.records.assign((size_t)nchans * gslots, 0);
     sb.meta.assign((size_t)nchans * sb.nblk * 2, 0);
     sb.skew.assign(sb.passes.size() * (size_t)ndm, 0);
@@ -358,7 +374,7 @@ struct SbArgs {
     int slot_chunks;          // 16-byte chunks per staged channel slot
     int raw_slot_bytes;       // raw path: bytes per raw channel slot
     int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
-    int first;                // 1: the launch's pass stores, 0: every pass adds into out
+    int first;                // 1: the launch's passes store, 0: every pass adds into out, 2: per pass (table flag)
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
 };
 
@@ -370,7 +386,7 @@ typedef unsigned long long sb_u64;     // one aligned register pair = two fp32 a
 // the consumers walk it with identical arithmetic.
 struct SbTile {
     int p, w, rot;            // cursor: pass, next tile index of this CTA within it (-1: pass not opened), list offset mod grid
-    int blk, beam, c_begin, c_end;
+    int blk, beam, c_begin, c_end, first;
     long long U0;
     const int32_t *skew;
 };
@@ -397,6 +413,7 @@ __device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
         if (t.U0 + SB_T <= (long long)__ldg(t.skew + d_first) || t.U0 >= (long long)__ldg(t.skew + d_last) + A.nsamp_out) continue;
         t.c_begin = P.c_begin;
         t.c_end = P.c_end;
+        t.first = P.first;
         return true;
     }
 }
@@ -603,7 +620,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         // are 16-byte aligned in the buffer too: one LDS.128 + one vector store / reduction per group.
         float *out = reinterpret_cast<float *>(A.out) + (size_t)t.beam * A.out_beam;
         const int d0 = t.blk * SB_ROWS + warp * SB_D;
-        const int first = A.first;
+        const int first = A.first == 2 ? t.first : A.first;
         const unsigned ep_u32 = (unsigned)__cvta_generic_to_shared(ep);
 #pragma unroll
         for (int j = 0; j < SB_D; ++j) {
@@ -736,7 +753,7 @@ bool subband_merges(const dedisp_plan *p) { return sb_merge_passes(p); }
 int subband_launches(const dedisp_plan *p, int resolved_kernel) {
     if (resolved_kernel != DEDISP_KERNEL_SUBBAND) return 1;
     const bool merged = sb_merge_passes(p);   // + a memset, which is not a kernel
-    return (merged ? 1 : (int)p->sb.passes.size()) + (p->dtype == DEDISP_U8 ? 1 : 0);
+    return (merged ? 1 : (int)p->sb.launch_begin.size() - 1) + (p->dtype == DEDISP_U8 ? 1 : 0);
 }
 
 cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out, void *d_out,
@@ -744,9 +761,10 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     const SubbandGeom &sb = p->sb;
     const long long nsamp_in = nsamp_out + p->maxshift;
     const int npass = (int)sb.passes.size();
-    const int pass_hi = run.pass_hi < 0 ? npass : run.pass_hi;
+    const int nlaunch = (int)sb.launch_begin.size() - 1;     // == npass for plans with one DM range
+    const int pass_hi = run.pass_hi < 0 ? nlaunch : run.pass_hi;
     const int blk_lo = run.blk_lo, blk_hi = run.blk_hi < 0 ? sb.nblk : run.blk_hi;
-    const bool whole = run.pass_lo == 0 && pass_hi == npass && blk_lo == 0 && blk_hi == sb.nblk;
+    const bool whole = run.pass_lo == 0 && pass_hi == nlaunch && blk_lo == 0 && blk_hi == sb.nblk;
     SbArgs A;
     A.in_stride = in_stride;
     A.in_total = (long long)(p->nchans - 1) * in_stride + nsamp_in;
@@ -801,19 +819,20 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (e != cudaSuccess) return e;
     } else {
         for (int i = run.pass_lo; i < pass_hi; ++i) {
-            const int g = run.reverse ? npass - 1 - i : i;
-            const SubbandPass &ps = sb.passes[g];
-            A.pass_lo = g; A.pass_hi = g + 1;
-            A.first = sb.nranges == 1 ? i == 0 : ps.first;   // one range: any order, the first launched pass stores
-            if (run.pass_ready) {   // dedisp_execute_host: this pass's channel rows arrive on the copy stream
+            const int g = run.reverse ? nlaunch - 1 - i : i;          // launch g = passes [launch_begin[g], launch_begin[g + 1])
+            A.pass_lo = sb.launch_begin[g]; A.pass_hi = sb.launch_begin[g + 1];
+            A.first = sb.nranges == 1 ? i == 0 : 2;   // one range: any order, the first launched pass stores; else per pass
+            if (run.pass_ready) {   // dedisp_execute_host (one DM range): this pass's channel rows arrive on the copy stream
                 e = cudaStreamWaitEvent(st, run.pass_ready[g], 0);
                 if (e != cudaSuccess) return e;
             }
-            e = launch(tiles_of(ps));
+            long long tiles = 0;
+            for (int q = A.pass_lo; q < A.pass_hi; ++q) tiles += tiles_of(sb.passes[q]);
+            e = launch(tiles);
             if (e != cudaSuccess) return e;
         }
     }
-    if (p->dtype == DEDISP_U8 && pass_hi == npass) {   // last pass done for these rows
+    if (p->dtype == DEDISP_U8 && pass_hi == nlaunch) {   // last pass done for these rows
         const int d0 = std::min(p->ndm, blk_lo * SB_ROWS), d1 = std::min(p->ndm, blk_hi * SB_ROWS);
         for (int r0 = d0; r0 < d1; r0 += 32768) {   // grid.y <= 65535
             dim3 grid((unsigned)((nsamp_out + 255) / 256), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
