@@ -17,7 +17,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dedisp_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle_dedisp.so")
+_SRC_CT = os.path.join(_HERE, "corner_turn_oracle.cpp")
+_LIB_CT = os.path.join(_HERE, "liboracle_corner_turn.so")
 _lib = None
+_lib_ct = None
 
 
 def build(force: bool = False) -> str:
@@ -26,6 +29,8 @@ def build(force: bool = False) -> str:
         cmd = ["g++", "-O3", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared",
                "-o", _LIB, _SRC]
         subprocess.run(cmd, check=True)
+    if force or not os.path.exists(_LIB_CT) or os.path.getmtime(_LIB_CT) < os.path.getmtime(_SRC_CT):
+        subprocess.run(["g++", "-O3", "-std=c++17", "-fPIC", "-shared", "-o", _LIB_CT, _SRC_CT], check=True)
     return _LIB
 
 
@@ -110,3 +115,21 @@ def dedisperse(nchans, fch1, foff, tsamp, dm_list, data: np.ndarray, nsamp_out: 
     if rc:
         raise ValueError(f"oracle dedisperse rc={rc}")
     return res
+
+
+def unpack_time_major(raw: np.ndarray, nchans: int, nbits: int) -> np.ndarray:
+    """``raw[nsamp][row_bytes]`` uint8 (time-major, ``nbits``-bit samples, first channel in the least
+    significant bits) -> channel-major uint8 ``[nchans][nsamp]`` (oracle/corner_turn_oracle.cpp)."""
+    global _lib_ct
+    if _lib_ct is None:
+        build()
+        _lib_ct = ctypes.CDLL(_LIB_CT)
+        _lib_ct.oracle_unpack_time_major.argtypes = [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_int,
+                                                      ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong]
+        _lib_ct.oracle_unpack_time_major.restype = ctypes.c_int
+    assert raw.ndim == 2 and raw.dtype == np.uint8 and raw.flags.c_contiguous
+    out = np.empty((nchans, raw.shape[0]), dtype=np.uint8)
+    rc = _lib_ct.oracle_unpack_time_major(raw.ctypes.data, raw.shape[1], raw.shape[0], nchans, nbits, out.ctypes.data, raw.shape[0])
+    if rc:
+        raise ValueError(f"oracle_unpack_time_major rc={rc}")
+    return out

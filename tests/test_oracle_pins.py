@@ -220,3 +220,36 @@ def test_float_sequential_diagnostic_inside_tolerance():
     o, a = oracle.dedisperse(*plan_of(cfg), dms, x, 512)
     s = oracle.dedisperse(*plan_of(cfg), dms, x, 512, seq_f32=True)
     assert np.max(np.abs(s - o) / a) < 1e-6
+
+
+# ---- corner turn + unpack in front of the hot path (oracle/corner_turn_oracle.cpp)
+def test_unpack_time_major_hand_packed_bytes():
+    """Hand-packed rows, reading R15: first channel in the least significant bits."""
+    # 4-bit, 4 channels, 2 time samples: t0 = (1, 2, 3, 4) -> bytes 0x21 0x43; t1 = (15, 0, 9, 6) -> 0x0F 0x69
+    raw = np.array([[0x21, 0x43], [0x0F, 0x69]], dtype=np.uint8)
+    assert oracle.unpack_time_major(raw, 4, 4).tolist() == [[1, 15], [2, 0], [3, 9], [4, 6]]
+    # 2-bit, 4 channels per byte: (3, 0, 1, 2) -> 0b10_01_00_11 = 0x93
+    assert oracle.unpack_time_major(np.array([[0x93]], dtype=np.uint8), 4, 2).tolist() == [[3], [0], [1], [2]]
+    # 1-bit, 8 channels per byte: channels 0, 3, 7 set -> 0b1000_1001 = 0x89; a pad byte is ignored
+    assert oracle.unpack_time_major(np.array([[0x89, 0xFF]], dtype=np.uint8), 8, 1).ravel().tolist() == [1, 0, 0, 1, 0, 0, 0, 1]
+    # 8-bit is a plain transpose
+    raw = np.arange(12, dtype=np.uint8).reshape(3, 4)
+    assert np.array_equal(oracle.unpack_time_major(raw, 4, 8), raw.T)
+
+
+@pytest.mark.parametrize("nbits", [1, 2, 4, 8])
+def test_unpack_time_major_vs_numpy_and_round_trip(nbits):
+    """Independent statement with numpy: unpackbits(bitorder='little') regrouped nbits at a time; and a
+    pack -> unpack round trip from known channel-major values, with padded rows."""
+    rng = np.random.default_rng(40 + nbits)
+    nchans, nsamp, pad = 48, 37, 5
+    row_bytes = nchans * nbits // 8 + pad
+    raw = rng.integers(0, 256, size=(nsamp, row_bytes), dtype=np.uint8)
+    bits = np.unpackbits(raw[:, : nchans * nbits // 8], axis=1, bitorder="little").reshape(nsamp, nchans, nbits)
+    want = (bits * (1 << np.arange(nbits))).sum(axis=2).astype(np.uint8).T
+    assert np.array_equal(oracle.unpack_time_major(raw, nchans, nbits), want)
+    vals = rng.integers(0, 1 << nbits, size=(nchans, nsamp), dtype=np.uint8)          # [c][t]
+    vbits = ((vals.T[:, :, None] >> np.arange(nbits)) & 1).astype(np.uint8).reshape(nsamp, nchans * nbits)
+    packed = np.packbits(vbits, axis=1, bitorder="little")
+    packed = np.concatenate([packed, np.full((nsamp, pad), 0xAA, dtype=np.uint8)], axis=1)
+    assert np.array_equal(oracle.unpack_time_major(np.ascontiguousarray(packed), nchans, nbits), vals)
