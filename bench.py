@@ -11,6 +11,7 @@ that carries BASELINE.json's roofline target. Metric: Gadds/s, one add per (DM, 
 from __future__ import annotations
 
 import argparse
+from dataclasses import replace
 import json
 import os
 import subprocess
@@ -511,6 +512,82 @@ def _c5_line(args, cfg, plan, hbm_gbs, sm_max_mhz, peak_src, value, total_ms, st
     print(json.dumps(line), flush=True)
 
 
+def run_time_major(args, cfg):
+    """the same workload fed TIME-major with nbits-bit packed samples through
+    dedisp_execute_time_major (corner turn + unpack fused into the staging step). value: input resident;
+    e2e: pinned host block -> H2D -> execute -> D2H of the result. 1 GPU, one beam."""
+    import torch
+
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import synth
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product has no CPU path"
+    assert cfg.dtype == "u8", "time-major input is integer data: use --config c2 or c5"
+    nbits = args.time_major
+    hbm_gbs, sm_max_mhz, peak_src = _peaks()
+    plan = P.Plan.from_config(cfg, time_major=True)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    x, _ = synth.make_input(cfg, plan.shifts(), nsamp_in, device="cuda")          # [c][t] u8
+    q = (x >> (8 - nbits)).t().contiguous()                                       # [t][c], values < 2**nbits
+    per = 8 // nbits
+    packed = (q.view(nsamp_in, cfg.nchans // per, per).to(torch.int32) << (nbits * torch.arange(per, device="cuda", dtype=torch.int32))).sum(dim=2).to(torch.uint8)
+    row = (packed.shape[1] + 15) // 16 * 16
+    raw = torch.zeros((nsamp_in, row), dtype=torch.uint8, device="cuda")
+    raw[:, :packed.shape[1]] = packed
+    del x, q, packed
+    out = plan.alloc_out(cfg.nsamp_out)
+    adds = cfg.ndm * cfg.nchans * cfg.nsamp_out
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        plan.execute_time_major(raw, nbits, cfg.nsamp_out, out)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    torch.cuda.synchronize()
+    sampler.start()
+    for a, b in evs:
+        a.record(stream)
+        plan.execute_time_major(raw, nbits, cfg.nsamp_out, out)
+        b.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    total_ms = evs[0][0].elapsed_time(evs[-1][1])
+    steps = sorted(a.elapsed_time(b) for a, b in evs)
+    step_ms = sum(steps) / len(steps)
+    e2e = None
+    if not args.no_e2e:
+        h_raw = raw.cpu().pin_memory()
+        h_out = torch.empty((cfg.ndm, cfg.nsamp_out), dtype=torch.int32, pin_memory=True)
+        esteps = max(1, min(args.steps, args.e2e_steps))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(esteps):
+            raw.copy_(h_raw, non_blocking=True)
+            plan.execute_time_major(raw, nbits, cfg.nsamp_out, out)
+            h_out.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        et = time.perf_counter() - t0
+        e2e = {"value": adds * esteps / et / 1e9, "unit": UNIT, "h2d_bytes_per_step": h_raw.numel(),
+               "d2h_bytes_per_step": h_out.numel() * 4, "steps": esteps, "ms_per_step": 1e3 * et / esteps,
+               "api": "pinned host block -> H2D -> dedisp_execute_time_major -> D2H"}
+    peak = add_peak(sm_max_mhz)
+    achieved = adds / (step_ms * 1e-3) / 1e9
+    bytes_once = raw.numel() + cfg.ndm * cfg.nsamp_out * 4
+    line = {"metric": METRIC, "value": adds * args.steps / (total_ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "i32", "data": "synthetic",
+            "config": {"workload": cfg.name + f"_time_major_{nbits}bit", "nchans": cfg.nchans, "ndm": cfg.ndm, "nsamp_out": cfg.nsamp_out,
+                       "nsamp_in": nsamp_in, "in_dtype": f"u{nbits} packed, time-major [t][c], row {row} bytes", "kernel": "subband",
+                       "passes": plan.num_subbands(), "l2": "out larger than L2, no flush"},
+            "real_time_factor": cfg.nsamp_out * cfg.tsamp / (total_ms / args.steps * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_execute * args.steps,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak, "traffic": None,
+                         "kernel": "dedisp_subband_kernel (time-major staging)", "launches_per_step": plan.launches_per_execute,
+                         "peak_source": f"148 SMs x 128 lanes x sm_max_mhz ({peak_src} MEASURED_PEAKS.json clock)",
+                         "hbm_bytes_once": bytes_once, "ms_median": steps[len(steps) // 2], "ms_best": steps[0]},
+            "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+
+
 def run_paper_sweep(args):
     """the paper's Fig. 4 regime (ndm = nchans) as a second workload; one
     JSON line per point, with the paper's own axis ("execution time as percentage of real-time")."""
@@ -564,6 +641,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=3.0, help="cpu_baseline: oracle seconds per timed call")
     ap.add_argument("--no-others", action="store_true", help="skip the c2/c4/c5 block of the default line")
+    ap.add_argument("--time-major", type=int, default=0, choices=[0, 1, 2, 4, 8],
+                    help="feed the (u8) config time-major with this many bits per sample (dedisp_execute_time_major)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--stream-chunks", type=int, default=0, help="c5 e2e: chunks pushed (default: the config's 60)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -587,6 +666,8 @@ def main():
         run_paper_sweep(args)
     elif args.impl == "reference":
         run_reference(args, cfg)
+    elif args.time_major:
+        run_time_major(args, replace(cfg, nbeams=1, nchunks=1))
     elif args.config == "c5":
         run_c5_stream(args, cfg)
     else:

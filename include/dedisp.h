@@ -53,7 +53,10 @@ enum dedisp_kernel {
 
 enum dedisp_plan_flags {
     DEDISP_PLAN_DEFAULT = 0,
-    DEDISP_PLAN_HOST_ONLY = 1  /* build host tables only; no CUDA call is made; execute -> EUNSUPPORTED */
+    DEDISP_PLAN_HOST_ONLY = 1, /* build host tables only; no CUDA call is made; execute -> EUNSUPPORTED */
+    DEDISP_PLAN_TIME_MAJOR = 2 /* the plan will be fed TIME-major packed input through dedisp_execute_time_major:
+                                  in_dtype must be DEDISP_U8 and nchans a multiple of 16 (else EINVAL); sub-bands
+                                  are cut at multiples of 16 channels. Channel-major calls stay available. */
 };
 
 /* ---- subsystem (2): shift-table builder ("the shifting value
@@ -88,6 +91,20 @@ int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1_mhz, doubl
  * SUBBAND kernel's staging step; there is no scratch copy of the input.) EINVAL: NULLs, nsamp_out < 1. */
 int dedisp_execute(dedisp_plan *plan, const void *d_in, long long nsamp_out, void *d_out,
                    void *stream);
+
+/* Fused corner turn + unpack (the stage in front of the
+ * "real-time dispersion searches" delivers time-major data; the kernel wants "cache-lines of
+ * constant frequency, contiguous time"). d_in is TIME-major (sigproc filterbank order): row t, 0 <= t <
+ * nsamp_out + maxshift, holds all channels of time sample t as nbits-wide unsigned integers, nbits in
+ * {1, 2, 4, 8}; sample (t, c) occupies bits [(c*nbits) mod 8, +nbits) of byte (c*nbits)/8 of the row (first
+ * channel in the least significant bits). Rows are row_bytes apart. The SUBBAND kernel's producer warps
+ * read these rows directly and write fp32 channel windows into the pipeline ring: no transposed or
+ * unpacked copy of the input exists in HBM. d_out: [ndm][nsamp_out] int32, exact.
+ * The plan must have been created with DEDISP_PLAN_TIME_MAJOR and admit the SUBBAND kernel
+ * (EUNSUPPORTED otherwise). EINVAL: NULLs, nbits not in {1,2,4,8}, row_bytes < nchans*nbits/8, d_in or
+ * row_bytes not 16-byte aligned. Allocates nothing; asynchronous on `stream`. */
+int dedisp_execute_time_major(dedisp_plan *plan, const void *d_in, int nbits, long long row_bytes,
+                              long long nsamp_out, void *d_out, void *stream);
 
 /* Same with explicit row strides in ELEMENTS (in_stride >= nsamp_out + maxshift, out_stride >=
  * nsamp_out), else EINVAL. Any base address and any stride are correct; a 16-byte-aligned d_in and

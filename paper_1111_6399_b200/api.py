@@ -19,6 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 U8, F16, F32 = 0, 1, 2
 KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND = 0, 1, 2, 3
 PLAN_HOST_ONLY = 1
+PLAN_TIME_MAJOR = 2
 
 DTYPE_CODE = {"u8": U8, "f16": F16, "f32": F32}
 _TORCH_IN = {U8: torch.uint8, F16: torch.float16, F32: torch.float32}
@@ -27,7 +28,7 @@ _TORCH_OUT = {U8: torch.int32, F16: torch.float32, F32: torch.float32}
 # every symbol include/dedisp.h declares (tests check the library exports them all)
 SYMBOLS = (
     "dedisp_shift_table_host", "dedisp_plan_create", "dedisp_plan_create_ex", "dedisp_execute",
-    "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_plan_destroy", "dedisp_plan_max_shift",
+    "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_execute_time_major", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
     "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_error_string",
@@ -58,6 +59,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_execute_strided.argtypes = [vp, vp, c_ll, c_ll, vp, c_ll, vp]
         L.dedisp_execute_batched.argtypes = [vp, c_int, vp, c_ll, c_ll, c_ll, vp, c_ll, c_ll, vp]
         L.dedisp_execute_host.argtypes = [vp, vp, c_ll, vp, vp]
+        L.dedisp_execute_time_major.argtypes = [vp, vp, c_int, c_ll, c_ll, vp, vp]
         L.dedisp_plan_destroy.argtypes = [vp]
         L.dedisp_plan_max_shift.argtypes = [vp]
         L.dedisp_plan_max_shift.restype = c_ll
@@ -111,12 +113,13 @@ def _stream_ptr(stream) -> int:
 class Plan:
     """``dedisp_plan``: shift table + kernel metadata for one (band, sampling, DM list, dtype)."""
 
-    def __init__(self, nchans, fch1, foff, tsamp, dm_list, dtype, host_only: bool = False):
+    def __init__(self, nchans, fch1, foff, tsamp, dm_list, dtype, host_only: bool = False, time_major: bool = False):
         self._h = ctypes.c_void_p()
         self.dtype = DTYPE_CODE[dtype] if isinstance(dtype, str) else int(dtype)
         dm, dmp = _dm(dm_list)
+        flags = (PLAN_HOST_ONLY if host_only else 0) | (PLAN_TIME_MAJOR if time_major else 0)
         rc = lib().dedisp_plan_create_ex(ctypes.byref(self._h), int(nchans), float(fch1), float(foff), float(tsamp),
-                                         dmp, dm.size, self.dtype, PLAN_HOST_ONLY if host_only else 0)
+                                         dmp, dm.size, self.dtype, flags)
         if rc:
             self._h = ctypes.c_void_p()
             raise DedispError(rc, "dedisp_plan_create")
@@ -124,8 +127,8 @@ class Plan:
         self.max_shift = int(lib().dedisp_plan_max_shift(self._h))
 
     @classmethod
-    def from_config(cls, cfg, host_only: bool = False) -> "Plan":
-        return cls(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), cfg.dtype, host_only)
+    def from_config(cls, cfg, host_only: bool = False, time_major: bool = False) -> "Plan":
+        return cls(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), cfg.dtype, host_only, time_major)
 
     def _check(self, rc, what):
         if rc:
@@ -201,6 +204,18 @@ class Plan:
                                               nsamp_out, d_out.data_ptr(),
                                               d_out.stride(0) if self.ndm > 1 else d_out.shape[1], st)
         self._check(rc, "dedisp_execute")
+        return d_out
+
+    def execute_time_major(self, d_raw: torch.Tensor, nbits: int, nsamp_out: int, d_out: Optional[torch.Tensor] = None, stream=None):
+        """``dedisp_execute_time_major``: ``d_raw[nsamp_out + max_shift][row_bytes]`` uint8 on the device, time-major,
+        ``nbits``-bit samples packed first-channel-in-the-low-bits; returns int32 ``[ndm][nsamp_out]``."""
+        assert d_raw.is_cuda and d_raw.dtype == torch.uint8 and d_raw.dim() == 2 and d_raw.stride(1) == 1
+        assert d_raw.shape[0] >= nsamp_out + self.max_shift
+        if d_out is None:
+            d_out = self.alloc_out(nsamp_out, None, d_raw.device)
+        assert d_out.is_cuda and d_out.dtype == torch.int32 and d_out.is_contiguous()
+        self._check(lib().dedisp_execute_time_major(self._h, d_raw.data_ptr(), int(nbits), d_raw.stride(0), nsamp_out,
+                                                    d_out.data_ptr(), _stream_ptr(stream)), "dedisp_execute_time_major")
         return d_out
 
     def execute_host(self, h_in: torch.Tensor, nsamp_out: int, h_out: Optional[torch.Tensor] = None, stream=None):

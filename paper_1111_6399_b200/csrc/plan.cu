@@ -64,6 +64,7 @@ int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1, double fo
     *plan = nullptr;
     if (in_dtype != DEDISP_U8 && in_dtype != DEDISP_F16 && in_dtype != DEDISP_F32) return DEDISP_EINVAL;
     if (nchans < 1 || ndm < 1 || !h_dm_list) return DEDISP_EINVAL;
+    if ((flags & DEDISP_PLAN_TIME_MAJOR) && (in_dtype != DEDISP_U8 || nchans % 16 != 0)) return DEDISP_EINVAL;
     if ((double)nchans * (double)ndm > 2.0e9) return DEDISP_EUNSUPPORTED;
     dedisp_plan *p = new (std::nothrow) dedisp_plan();
     if (!p) return DEDISP_ENOMEM;
@@ -71,6 +72,7 @@ int dedisp_plan_create_ex(dedisp_plan **plan, int nchans, double fch1, double fo
     try {
         p->nchans = nchans; p->ndm = ndm; p->dtype = in_dtype;
         p->fch1 = fch1; p->foff = foff; p->tsamp = tsamp; p->flags = flags;
+        p->time_major = (flags & DEDISP_PLAN_TIME_MAJOR) != 0;
         p->dm.assign(h_dm_list, h_dm_list + ndm);
         p->shifts.resize((size_t)nchans * ndm);
         rc = build_shift_table(nchans, fch1, foff, tsamp, p->dm.data(), ndm, p->shifts.data(), &p->maxshift);
@@ -114,6 +116,21 @@ int dedisp_plan_create(dedisp_plan **plan, int nchans, double fch1, double foff,
 int dedisp_execute_strided(dedisp_plan *p, const void *d_in, long long in_stride, long long nsamp_out,
                            void *d_out, long long out_stride, void *stream) {
     return execute_impl(p, d_in, in_stride, nsamp_out, d_out, out_stride, Batch(), (cudaStream_t)stream);
+}
+
+int dedisp_execute_time_major(dedisp_plan *p, const void *d_in, int nbits, long long row_bytes, long long nsamp_out,
+                              void *d_out, void *stream) {
+    if (!p || !d_in || !d_out || nsamp_out < 1) return DEDISP_EINVAL;
+    if (nbits != 1 && nbits != 2 && nbits != 4 && nbits != 8) return DEDISP_EINVAL;
+    if (row_bytes * 8 < (long long)p->nchans * nbits || (row_bytes & 15) != 0 || ((uintptr_t)d_in & 15) != 0) return DEDISP_EINVAL;
+    if (p->flags & DEDISP_PLAN_HOST_ONLY) return DEDISP_EUNSUPPORTED;
+    if (!p->time_major || !p->sb.ok || p->sb.cb != 16) return DEDISP_EUNSUPPORTED;   // corner turn lives in the SUBBAND staging step
+    if (nsamp_out + p->maxshift >= (1ll << 40)) return DEDISP_EUNSUPPORTED;
+    SbRun run;
+    run.tm_bits = nbits;
+    const cudaError_t e = launch_subband(p, d_in, row_bytes, nsamp_out, d_out, nsamp_out, Batch(), (cudaStream_t)stream, run);
+    if (e != cudaSuccess) return fail_cuda(p, e, "kernel launch");
+    return DEDISP_OK;
 }
 
 int dedisp_execute(dedisp_plan *p, const void *d_in, long long nsamp_out, void *d_out, void *stream) {

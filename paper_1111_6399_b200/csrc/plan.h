@@ -83,6 +83,7 @@ struct SbRun {
     int blk_lo = 0, blk_hi = -1;       // DM blocks (-1: all)
     bool reverse = false;              // run the passes last sub-band first
     const cudaEvent_t *pass_ready = nullptr;
+    int tm_bits = 0;                   // != 0: d_in is TIME-major, tm_bits (1/2/4/8) per sample, in_stride = bytes per time sample
 };
 
 struct SubbandGeom {
@@ -112,6 +113,7 @@ struct dedisp_plan {
     int nchans = 0, ndm = 0, dtype = 0;
     double fch1 = 0, foff = 0, tsamp = 0;
     unsigned flags = 0;
+    bool time_major = false;          // DEDISP_PLAN_TIME_MAJOR: sub-bands cut at multiples of 16 channels
     std::vector<double> dm;
     std::vector<int32_t> shifts;  // [c][d]
     long long maxshift = 0;

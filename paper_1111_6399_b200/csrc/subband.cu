@@ -185,6 +185,10 @@ void subband_build(dedisp_plan *p) {
                 }
                 good = lo;
             }
+            if (p->time_major && good < nchans) {   // time-major input: sub-bands (and so stages) start at multiples of 16 channels
+                good = cb + (good - cb) / 16 * 16;
+                if (good == cb) { sb = SubbandGeom(); return; }
+            }
             SubbandPass ps;
             ps.c_begin = cb;
             ps.c_end = good;
@@ -198,7 +202,7 @@ void subband_build(dedisp_plan *p) {
         // whole sweep over out (c3: 8 channels, 1.0 ms), so share the channels of the last two evenly
         if (cut.size() >= 2) {
             SubbandPass &u = cut[cut.size() - 2], &v = cut.back();
-            const int mid = (u.c_begin + v.c_end) / 2;
+            const int mid = p->time_major ? (u.c_begin + v.c_end) / 32 * 16 : (u.c_begin + v.c_end) / 2;
             if (v.c_end - v.c_begin < (u.c_end - u.c_begin) / 2 && mid > u.c_begin && mid <= u.c_end &&
                 pass_geometry(p, mid, v.c_end, pick_ref(p, mid, v.c_end), false, b0, b1)) {
                 u.c_end = mid;
@@ -443,9 +447,20 @@ template <> __device__ __forceinline__ float sb_to_f32<__half>(__half v) { retur
 // windows are TMA-copied as raw bytes (from the 16-byte boundary below their first sample) into a raw
 // buffer, and the four producer warps convert them to fp32 into the ring - no pre-pass over the input
 // and no fp32 copy of it in HBM.
-template <typename TIN, bool RAW>
+//
+// MODE 0: direct, 1: raw, 2..5: TIME-MAJOR packed input with 8 / 4 / 2 / 1 bits per sample (SURVEY.md §8(f)
+// rank 2: corner turn + unpack fused into the staging step; PAPER.md:26 names the stage in front of the
+// dispersion search, PAPER.md:42 the channel-major view this kernel wants). Row t of the input holds all
+// channels of time sample t, first channel in the least significant bits; the plan cuts its sub-bands
+// at multiples of 16 channels and a stage is exactly 16 channels, so a stage reads 2*nbits contiguous
+// bytes per time sample. The four producer warps walk the union of the stage's windows one time sample
+// per lane, load those bytes straight from global memory, and scatter the 16 values as fp32 into the 16
+// channel windows of the ring: the corner turn costs no extra pass over the input and no staging buffer.
+template <typename TIN, int MODE>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
-    typedef float OutT;
+    constexpr bool RAW = MODE == 1;
+    constexpr int TMB = MODE == 2 ? 8 : MODE == 3 ? 4 : MODE == 4 ? 2 : MODE == 5 ? 1 : 0;   // time-major: bits per sample
+    constexpr bool CONV = RAW || TMB != 0;                                                   // producer warps write the ring
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const unsigned slot_bytes = (unsigned)A.slot_chunks * 16;
@@ -462,7 +477,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned raw_base = sdata_base + ep_off + SB_WARPS * SB_EP_WORDS * 4;
     if (tid == 0) {
 #pragma unroll
-        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, RAW ? 4 : 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
+        for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, CONV ? 4 : 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
         sb_mbar_init(bar_raw_full, 1);
         sb_mbar_init(bar_raw_empty, 4);
     }
@@ -473,7 +488,74 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 
     if (warp >= SB_WARPS) {
         // ---------------- producer warpgroup: its first warp fills the ring
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(SbRegs<RAW>::producer));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(SbRegs<CONV>::producer));
+        if constexpr (TMB != 0) {
+            const int pw = warp - SB_WARPS;
+            const unsigned char *inb = reinterpret_cast<const unsigned char *>(A.in);
+            while (sb_next_tile(A, t)) {
+                const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
+                for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {   // CB == 16, c0 % 16 == 0 (plan built with DEDISP_PLAN_TIME_MAJOR)
+                    const int buf = it % SB_STAGES, k = it / SB_STAGES;
+                    const unsigned full = bar_full + 8u * buf;
+                    const int n = min(CB, t.c_end - c0);
+                    // lane j < n: window of channel c0 + j in time samples [e0, e0 + nw)
+                    const int2 mt = lane < n ? __ldg(meta + c0 + lane) : make_int2(0, 0);
+                    const long long e0 = t.U0 + mt.x;
+                    const int nw = 4 * mt.y;
+                    long long t_lo = lane < n ? e0 : (1ll << 62), t_hi = lane < n ? e0 + nw : -(1ll << 62);
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        t_lo = min(t_lo, __shfl_xor_sync(0xffffffffu, t_lo, o));
+                        t_hi = max(t_hi, __shfl_xor_sync(0xffffffffu, t_hi, o));
+                    }
+                    if (k > 0) sb_mbar_wait_sleep(bar_empty + 8u * buf, (unsigned)((k - 1) & 1));
+                    if (pw == 0 && lane == 0) {   // the stage's records: n x SB_WARPS, contiguous
+                        sb_mbar_expect_tx(full, (unsigned)n * SB_REC_STRIDE);
+                        sb_bulk_g2s(srec_base + buf * CB * SB_REC_STRIDE, A.records + ((size_t)t.blk * A.nchans + c0) * SB_WARPS, (unsigned)n * SB_REC_STRIDE, full);
+                    }
+                    // lane j keeps channel j's slot address minus its window start, and its window as [lo, lo + nw)
+                    // in samples relative to the union's first sample
+                    const int lo = (int)(e0 - t_lo);
+                    const unsigned sbase = sdata_base + buf * stage_bytes + lane * slot_bytes - 4u * (unsigned)lo;
+                    const size_t col = (size_t)c0 * TMB / 8;                  // byte of channel c0 in a row
+                    constexpr int NW = TMB == 8 ? 4 : TMB == 4 ? 2 : 1;       // 32-bit words per row: 16 channels
+                    constexpr int NB = TMB == 8 ? 2 : 4;                      // rows per lane in flight: all loads first, then the scatter
+                    for (long long tb = t_lo + 32 * NB * pw; tb < t_hi; tb += 128 * NB) {   // 32 * NB time samples per warp and step
+                        unsigned w[NB][NW];
+#pragma unroll
+                        for (int r = 0; r < NB; ++r) {
+                            const long long ts = tb + 32 * r + lane;
+#pragma unroll
+                            for (int q = 0; q < NW; ++q) w[r][q] = 0u;
+                            if (ts >= 0 && ts < A.in_total && ts < t_hi) {
+                                const unsigned char *src = inb + (size_t)ts * A.in_stride + col;
+                                if constexpr (TMB == 8) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src)); w[r][0] = v.x; w[r][1] = v.y; w[r][2] = v.z; w[r][3] = v.w; }
+                                else if constexpr (TMB == 4) { const uint2 v = __ldg(reinterpret_cast<const uint2 *>(src)); w[r][0] = v.x; w[r][1] = v.y; }
+                                else if constexpr (TMB == 2) w[r][0] = __ldg(reinterpret_cast<const unsigned *>(src));
+                                else w[r][0] = __ldg(reinterpret_cast<const unsigned short *>(src));
+                            }
+                        }
+                        const int idx0 = (int)(tb - t_lo) + lane;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            constexpr unsigned per = 32 / TMB;                // samples per 32-bit word
+                            const int loj = __shfl_sync(0xffffffffu, lo, j);
+                            const int nj = __shfl_sync(0xffffffffu, nw, j);
+                            const unsigned bj = __shfl_sync(0xffffffffu, sbase, j) + 4u * (unsigned)idx0;
+#pragma unroll
+                            for (int r = 0; r < NB; ++r) {
+                                const unsigned x = (w[r][j / per] >> ((j % per) * TMB)) & ((1u << TMB) - 1u);
+                                if ((unsigned)(idx0 + 32 * r - loj) < (unsigned)nj)
+                                    asm volatile("st.shared.f32 [%0], %1;\n" ::"r"(bj + 128u * r), "f"((float)x) : "memory");
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) sb_mbar_arrive(full);
+                }
+            }
+            return;
+        }
         if constexpr (RAW) {
             const int pw = warp - SB_WARPS;
             constexpr long long ES = (long long)sizeof(TIN);
@@ -591,7 +673,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     }
 
     // ---------------- consumer warps
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SbRegs<RAW>::consumer));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SbRegs<CONV>::consumer));
     const unsigned sdata_u32 = sdata_base + 4u * SB_K * lane;
     float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * SB_EP_WORDS;
     while (sb_next_tile(A, t)) {
@@ -709,12 +791,20 @@ cudaError_t subband_upload(dedisp_plan *p) {
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_skew, sb.skew.data(), sb.skew.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
     switch (p->dtype) {
-        case DEDISP_U8: return cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
-        case DEDISP_F16: return cudaFuncSetAttribute(dedisp_subband_kernel<__half, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+        case DEDISP_U8:
+            e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+            if (e == cudaSuccess && p->time_major) {   // time-major launches use the direct path's layout (no raw buffer)
+                e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+            }
+            return e;
+        case DEDISP_F16: return cudaFuncSetAttribute(dedisp_subband_kernel<__half, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
         default: break;
     }
-    e = cudaFuncSetAttribute(dedisp_subband_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+    e = cudaFuncSetAttribute(dedisp_subband_kernel<float, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<float, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
     return e;
 }
 
@@ -767,10 +857,10 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     const bool whole = run.pass_lo == 0 && pass_hi == nlaunch && blk_lo == 0 && blk_hi == sb.nblk;
     SbArgs A;
     A.in_stride = in_stride;
-    A.in_total = (long long)(p->nchans - 1) * in_stride + nsamp_in;
+    A.in_total = run.tm_bits ? nsamp_in : (long long)(p->nchans - 1) * in_stride + nsamp_in;   // time-major: rows (time samples) of in_stride bytes
     A.in_beam = b.in_stride;
     cudaError_t e;
-    const bool raw = sb_raw_path(p, d_in, in_stride, b);
+    const bool raw = run.tm_bits == 0 && sb_raw_path(p, d_in, in_stride, b);
     A.in = d_in;
     A.out = d_out;
     A.out_stride = out_stride;
@@ -789,6 +879,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     A.slot_chunks = sb.slot_chunks;
     A.raw_slot_bytes = sb.raw_slot_bytes;
     A.cb = raw ? sb.cb_raw : sb.cb;
+    if (run.tm_bits && (A.cb != 16 || !p->time_major)) return cudaErrorInvalidValue;
     auto tiles_of = [&](const SubbandPass &ps) -> long long {
         const long long nb = std::min(blk_hi, ps.blk_end) - std::max(blk_lo, ps.blk_begin);
         return nb <= 0 ? 0 : nb * ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * b.n;
@@ -798,10 +889,14 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (tiles >= (1ll << 31)) return cudaErrorInvalidValue;
         const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, p->sm_count));
         // u8 plans too accumulate fp32 sums (exact, checked at plan build) in place; converted after the last pass
-        if (!raw) dedisp_subband_kernel<float, false><<<grid, SB_THREADS, sb.smem, st>>>(A);
-        else if (p->dtype == DEDISP_U8) dedisp_subband_kernel<uint8_t, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
-        else if (p->dtype == DEDISP_F16) dedisp_subband_kernel<__half, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
-        else dedisp_subband_kernel<float, true><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
+        if (run.tm_bits == 8) dedisp_subband_kernel<uint8_t, 2><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (run.tm_bits == 4) dedisp_subband_kernel<uint8_t, 3><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (run.tm_bits == 2) dedisp_subband_kernel<uint8_t, 4><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (run.tm_bits == 1) dedisp_subband_kernel<uint8_t, 5><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (!raw) dedisp_subband_kernel<float, 0><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (p->dtype == DEDISP_U8) dedisp_subband_kernel<uint8_t, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
+        else if (p->dtype == DEDISP_F16) dedisp_subband_kernel<__half, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
+        else dedisp_subband_kernel<float, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
         return cudaGetLastError();
     };
     if (whole && sb_merge_passes(p)) {
