@@ -19,8 +19,11 @@ _SRC = os.path.join(_HERE, "dedisp_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle_dedisp.so")
 _SRC_CT = os.path.join(_HERE, "corner_turn_oracle.cpp")
 _LIB_CT = os.path.join(_HERE, "liboracle_corner_turn.so")
+_SRC_DET = os.path.join(_HERE, "detect_oracle.cpp")
+_LIB_DET = os.path.join(_HERE, "liboracle_detect.so")
 _lib = None
 _lib_ct = None
+_lib_det = None
 
 
 def build(force: bool = False) -> str:
@@ -31,6 +34,8 @@ def build(force: bool = False) -> str:
         subprocess.run(cmd, check=True)
     if force or not os.path.exists(_LIB_CT) or os.path.getmtime(_LIB_CT) < os.path.getmtime(_SRC_CT):
         subprocess.run(["g++", "-O3", "-std=c++17", "-fPIC", "-shared", "-o", _LIB_CT, _SRC_CT], check=True)
+    if force or not os.path.exists(_LIB_DET) or os.path.getmtime(_LIB_DET) < os.path.getmtime(_SRC_DET):
+        subprocess.run(["g++", "-O3", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_DET, _SRC_DET], check=True)
     return _LIB
 
 
@@ -133,3 +138,26 @@ def unpack_time_major(raw: np.ndarray, nchans: int, nbits: int) -> np.ndarray:
     if rc:
         raise ValueError(f"oracle_unpack_time_major rc={rc}")
     return out
+
+
+CAND_DTYPE = np.dtype([("dm_index", np.int32), ("width", np.int32), ("t", np.int64), ("snr", np.float64)])
+
+
+def detect(x: np.ndarray, nwidths: int, threshold: float, max_out: int = 1 << 20):
+    """Detection oracle (oracle/detect_oracle.cpp) on ``x[nrows][n]`` (int32 or float32): returns
+    (candidates as a CAND_DTYPE array in (row, width, t) order, total count)."""
+    global _lib_det
+    if _lib_det is None:
+        build()
+        _lib_det = ctypes.CDLL(_LIB_DET)
+        for f in (_lib_det.oracle_detect_i32, _lib_det.oracle_detect_f32):
+            f.argtypes = [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_double,
+                          ctypes.c_void_p, ctypes.c_longlong]
+            f.restype = ctypes.c_longlong
+    assert x.ndim == 2 and x.flags.c_contiguous and x.dtype in (np.int32, np.float32)
+    out = np.zeros(max_out, dtype=CAND_DTYPE)
+    fn = _lib_det.oracle_detect_i32 if x.dtype == np.int32 else _lib_det.oracle_detect_f32
+    n = fn(x.ctypes.data, x.shape[1], x.shape[0], x.shape[1], nwidths, float(threshold), out.ctypes.data, max_out)
+    if n < 0:
+        raise ValueError("oracle_detect: bad arguments")
+    return out[:min(n, max_out)], int(n)

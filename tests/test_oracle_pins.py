@@ -253,3 +253,53 @@ def test_unpack_time_major_vs_numpy_and_round_trip(nbits):
     packed = np.packbits(vbits, axis=1, bitorder="little")
     packed = np.concatenate([packed, np.full((nsamp, pad), 0xAA, dtype=np.uint8)], axis=1)
     assert np.array_equal(oracle.unpack_time_major(np.ascontiguousarray(packed), nchans, nbits), vals)
+
+
+# ---- detection behind the hot path (oracle/detect_oracle.cpp, reading R16)
+def test_detect_closed_forms():
+    # alternating +-1: mu = 0, var = 1; width 1: snr = x; width 2: every window sums to 0
+    n = 64
+    x = np.where(np.arange(n) % 2 == 0, 1, -1).astype(np.int32)[None, :]
+    c, cnt = oracle.detect(x, 2, 0.5)
+    assert cnt == n // 2 and set(c["width"]) == {1} and np.all(c["t"] % 2 == 0) and np.allclose(c["snr"], 1.0)
+    # a lone pulse of width 4 and height a on a zero row of length n: mu = 4a/n, var = 4a^2/n - mu^2;
+    # the matched window (w = 4 at the pulse start) has snr = (4a - 4 mu) / (sd * 2), the largest of all
+    n, a, t0 = 1000, 7, 123
+    x = np.zeros((1, n), dtype=np.int32)
+    x[0, t0:t0 + 4] = a
+    mu = 4 * a / n
+    sd = math.sqrt(4 * a * a / n - mu * mu)
+    c, cnt = oracle.detect(x, 5, 0.0)
+    best = c[np.argmax(c["snr"])]
+    assert (best["width"], best["t"]) == (4, t0)
+    assert best["snr"] == ((4 * a - 4 * mu) * (1.0 / (sd * math.sqrt(4.0))))
+    w8 = c[(c["width"] == 8) & (c["t"] == t0 - 2)][0]          # a width-8 window around the pulse sees the same sum
+    assert abs(w8["snr"] - (4 * a - 8 * mu) / (sd * math.sqrt(8.0))) < 1e-12
+    # constant rows have no variance and yield nothing; float rows likewise
+    assert oracle.detect(np.full((2, 50), 5, dtype=np.int32), 3, -1e9)[1] == 0
+    assert oracle.detect(np.full((2, 50), 0.25, dtype=np.float32), 3, -1e9)[1] == 0
+
+
+@pytest.mark.parametrize("dtype", [np.int32, np.float32])
+def test_detect_vs_numpy_brute_force(dtype):
+    """Every (row, w, t) recomputed with direct window sums (no doubling) in numpy; integer rows must agree
+    exactly, float rows to 1e-6 (fp32 window sums in another order)."""
+    rng = np.random.default_rng(77)
+    nrows, n, nwidths, thr = 3, 257, 4, 1.5
+    x = rng.integers(-50, 200, size=(nrows, n)).astype(dtype) if dtype == np.int32 else rng.standard_normal((nrows, n)).astype(dtype)
+    c, cnt = oracle.detect(x, nwidths, thr)
+    assert cnt == len(c) > 0
+    got = {(int(r["dm_index"]), int(r["width"]), int(r["t"])): float(r["snr"]) for r in c}
+    want = {}
+    for r in range(nrows):
+        row = x[r].astype(np.float64)
+        mu, var = row.mean(), (row * row).mean() - row.mean() ** 2
+        for k in range(nwidths):
+            w = 1 << k
+            for t in range(n - w + 1):
+                snr = (row[t:t + w].sum() - w * mu) / (math.sqrt(var) * math.sqrt(w))
+                if snr >= thr + 1e-6 or (snr >= thr - 1e-6 and (r, w, t) in got):
+                    want[(r, w, t)] = snr
+    assert set(got) == set(want)
+    tol = 0.0 if dtype == np.int32 else 1e-6
+    assert max(abs(got[k] - want[k]) for k in got) <= max(tol, 1e-12)
