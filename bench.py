@@ -588,6 +588,84 @@ def run_time_major(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def run_detect(args, cfg):
+    """dedisp_detect on the de-dispersed block of the config (c5: 32 beams x 1024 DMs x
+    32768 samples int32 = 4.3 GB; c3: 4096 x 131072 fp32 = 2.1 GB), which stays on the GPU. HBM-bound: the block is
+    read twice (row statistics, then boxcar + threshold); roofline = 2 x block bytes / measured HBM bandwidth."""
+    import ctypes
+    import torch
+
+    import paper_1111_6399_b200 as P
+    from paper_1111_6399_b200 import synth
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product has no CPU path"
+    hbm_gbs, _, _ = _peaks()
+    plan = P.Plan.from_config(cfg)
+    nsamp_in = cfg.nsamp_out + plan.max_shift
+    tab = plan.shifts()
+    if cfg.nbeams > 1:
+        x = torch.empty((cfg.nbeams, cfg.nchans, nsamp_in), dtype=torch.uint8, device="cuda")
+        for b in range(cfg.nbeams):
+            x[b], _ = synth.make_input(cfg, tab, nsamp_in, device="cuda", seed=cfg.seed * 1000003 + b * 101)
+        out = plan.execute(x, cfg.nsamp_out)
+    else:
+        x, _ = synth.make_input(cfg, tab, nsamp_in, device="cuda")
+        out = plan.execute(x, cfg.nsamp_out)
+    torch.cuda.synchronize()
+    del x
+    block = out.view(-1, cfg.nsamp_out)
+    rows, n = block.shape
+    nwidths, thr, max_cands = 6, 7.0, 1 << 20
+    L = P.lib()
+    work = torch.empty(int(L.dedisp_detect_workspace_bytes(rows)) // 8 + 1, dtype=torch.int64, device="cuda")
+    cands = torch.empty(max_cands * P.CAND_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def call():
+        rc = L.dedisp_detect(block.data_ptr(), int(block.dtype == torch.float32), rows, n, block.stride(0), nwidths, thr,
+                             cands.data_ptr(), max_cands, work.data_ptr(), ctypes.c_void_p(stream.cuda_stream))
+        assert rc == 0
+
+    for _ in range(args.warmup):
+        call()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    torch.cuda.synchronize()
+    sampler.start()
+    for a, b in evs:
+        a.record(stream)
+        call()
+        b.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    steps = sorted(a.elapsed_time(b) for a, b in evs)
+    step_ms = sum(steps) / len(steps)
+    total = int(work[0].item())
+    t0 = time.perf_counter()
+    esteps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(esteps):
+        got, tot = P.detect(block, nwidths, thr, max_cands)       # call + sync + candidates copied to the host
+    et = (time.perf_counter() - t0) / esteps
+    nbytes = rows * n * 4
+    algo = 2 * nbytes
+    line = {"metric": "detection throughput (de-dispersed samples/s)", "value": rows * n / (step_ms * 1e-3) / 1e9, "unit": "Gsamples/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "i32" if block.dtype == torch.int32 else "f32", "data": "synthetic",
+            "config": {"workload": cfg.name + "_detect", "rows": rows, "nsamp": n, "nwidths": nwidths, "threshold_sigma": thr,
+                       "candidates": total, "l2": "block larger than L2, no flush"},
+            "clocks": clocks,
+            "e2e": {"value": rows * n / et / 1e9, "unit": "Gsamples/s", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 8 + len(got) * P.CAND_DTYPE.itemsize, "ms_per_step": 1e3 * et,
+                    "api": "dedisp_detect on the resident block + D2H of the count and the candidate list"},
+            "gpu_launches": 2 * args.steps,
+            "roofline": {"bound": "hbm", "achieved": algo / (step_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                         "frac": algo / (step_ms * 1e-3) / 1e9 / hbm_gbs, "traffic": None,
+                         "kernel": "dedisp_detect_stats_kernel + dedisp_detect_boxcar_kernel", "algorithmic_bytes": algo,
+                         "ms_median": steps[len(steps) // 2], "ms_best": steps[0]},
+            "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+
+
 def run_paper_sweep(args):
     """the paper's Fig. 4 regime (ndm = nchans) as a second workload; one
     JSON line per point, with the paper's own axis ("execution time as percentage of real-time")."""
@@ -643,6 +721,7 @@ def main():
     ap.add_argument("--no-others", action="store_true", help="skip the c2/c4/c5 block of the default line")
     ap.add_argument("--time-major", type=int, default=0, choices=[0, 1, 2, 4, 8],
                     help="feed the (u8) config time-major with this many bits per sample (dedisp_execute_time_major)")
+    ap.add_argument("--detect", action="store_true", help="time dedisp_detect on the config's de-dispersed block (c3 or c5)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--stream-chunks", type=int, default=0, help="c5 e2e: chunks pushed (default: the config's 60)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -666,6 +745,8 @@ def main():
         run_paper_sweep(args)
     elif args.impl == "reference":
         run_reference(args, cfg)
+    elif args.detect:
+        run_detect(args, cfg)
     elif args.time_major:
         run_time_major(args, replace(cfg, nbeams=1, nchunks=1))
     elif args.config == "c5":

@@ -176,6 +176,34 @@ int dedisp_plan_get_geometry(const dedisp_plan *plan, int *h_out);
  * call did not take the slab-overlap path). For the tests that must know which path they exercised. */
 int dedisp_plan_last_host_slabs(const dedisp_plan *plan);
 
+/* ---- detection behind the hot path ("detect millisecond radio
+ * bursts ... in real-time", "detection of interesting signals"). The paper gives no algorithm;
+ * this is the build's own definition (reading R16), stated so that it can be checked exactly:
+ * for every row x[0..nsamp) of a de-dispersed block d_block[ndm][stride] (int32 if block_is_float == 0,
+ * else float32):
+ *   1. S1 = sum x, S2 = sum x^2 (exact 64-bit integers for int32 rows, double for float rows), mu = S1/nsamp,
+ *      var = S2/nsamp - mu*mu; rows with var <= 0 yield nothing;
+ *   2. boxcar sums of width w = 1, 2, 4, ..., 2^(nwidths-1) by doubling in the row's own arithmetic:
+ *      y_1 = x, y_2w[t] = y_w[t] + y_w[t + w], for windows that lie inside the row;
+ *   3. snr_w[t] = (double(y_w[t]) - w*mu) * (1 / (sqrt(var) * sqrt(w))), IEEE double, each operation rounded
+ *      (no contraction) - integer rows therefore give bit-identical values on any conforming machine;
+ *   4. every (row, w, t) with snr_w[t] >= threshold is appended, in no particular order, to d_cands (device,
+ *      capacity max_cands records; further ones are counted but not stored).
+ * d_work: device scratch of dedisp_detect_workspace_bytes(ndm) bytes, 8-byte aligned, owned by the caller;
+ * when the call's work on `stream` has completed its first 8 bytes hold the total number of candidates
+ * (unsigned 64-bit). Allocates nothing, asynchronous on `stream`. EINVAL: NULLs, ndm < 1 or > 65535,
+ * nsamp < 1, stride < nsamp, nwidths < 1 or > DEDISP_DETECT_MAX_WIDTHS. */
+#define DEDISP_DETECT_MAX_WIDTHS 8
+typedef struct dedisp_candidate {
+    int dm_index;     /* row of the block */
+    int width;        /* boxcar width w in samples */
+    long long t;      /* first sample of the window */
+    double snr;
+} dedisp_candidate;
+long long dedisp_detect_workspace_bytes(int ndm);
+int dedisp_detect(const void *d_block, int block_is_float, int ndm, long long nsamp, long long stride, int nwidths,
+                  double threshold, dedisp_candidate *d_cands, long long max_cands, void *d_work, void *stream);
+
 const char *dedisp_error_string(int code);
 const char *dedisp_last_cuda_error(const dedisp_plan *plan);
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_execute_time_major", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
-    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_error_string",
+    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_detect_workspace_bytes", "dedisp_detect", "dedisp_error_string",
     "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_release_after", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
@@ -71,6 +71,9 @@ def lib() -> ctypes.CDLL:
         L.dedisp_plan_set_pass_merge.argtypes = [vp, c_int]
         L.dedisp_plan_get_subbands.argtypes = [vp, ip]
         L.dedisp_plan_get_geometry.argtypes = [vp, ip]
+        L.dedisp_detect_workspace_bytes.argtypes = [c_int]
+        L.dedisp_detect_workspace_bytes.restype = c_ll
+        L.dedisp_detect.argtypes = [vp, c_int, c_int, c_ll, c_ll, c_int, c_dbl, vp, c_ll, vp, vp]
         L.dedisp_plan_verify_records.argtypes = [vp]
         L.dedisp_plan_verify_records.restype = c_ll
         L.dedisp_error_string.argtypes = [c_int]
@@ -300,3 +303,23 @@ class Stream:
             self.close()
         except Exception:
             pass
+
+
+CAND_DTYPE = np.dtype([("dm_index", np.int32), ("width", np.int32), ("t", np.int64), ("snr", np.float64)])
+
+
+def detect(block: torch.Tensor, nwidths: int, threshold: float, max_cands: int = 1 << 20, stream=None):
+    """``dedisp_detect`` on a de-dispersed block ``[ndm][nsamp]`` (int32 or float32, device). Returns
+    (candidates as a CAND_DTYPE numpy array, total count). Marshalling only: buffers, call, copy back."""
+    assert block.is_cuda and block.dim() == 2 and block.stride(1) == 1 and block.dtype in (torch.int32, torch.float32)
+    ndm, nsamp = block.shape
+    work = torch.empty(int(lib().dedisp_detect_workspace_bytes(ndm)) // 8 + 1, dtype=torch.int64, device=block.device)
+    cands = torch.empty(max(1, max_cands) * CAND_DTYPE.itemsize, dtype=torch.uint8, device=block.device)
+    rc = lib().dedisp_detect(block.data_ptr(), int(block.dtype == torch.float32), ndm, nsamp, block.stride(0), int(nwidths),
+                             float(threshold), cands.data_ptr(), int(max_cands), work.data_ptr(), _stream_ptr(stream))
+    if rc:
+        raise DedispError(rc, "dedisp_detect")
+    torch.cuda.synchronize(block.device)
+    total = int(work[0].item())
+    out = np.frombuffer(cands[:min(total, max_cands) * CAND_DTYPE.itemsize].cpu().numpy().tobytes(), dtype=CAND_DTYPE)
+    return out, total
