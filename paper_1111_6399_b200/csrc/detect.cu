@@ -9,8 +9,9 @@
 //   rounded operations (no contraction), so that integer rows give bit-identical S/N on CPU and GPU;
 //   every (row, w, t) with snr >= threshold is appended to a candidate list through one atomic counter.
 //
-// Two HBM-bound kernels: row statistics (one read of the block) and boxcar + threshold (one more read,
-// plus a halo of 2^(nwidths-1) - 1 samples per tile); roofline = 2 x block bytes / HBM bandwidth.
+// Two HBM-bound kernels: row statistics (one read of the block) and boxcar + threshold (one more read;
+// neighbouring warp segments overlap by the largest width, served by L1/L2); roofline = 2 x block bytes /
+// HBM bandwidth.
 #include <cstdint>
 #include <type_traits>
 
@@ -22,6 +23,9 @@ constexpr int DET_THREADS = 256;
 constexpr int DET_PER = 8;                          // samples per thread and tile
 constexpr int DET_TILE = DET_THREADS * DET_PER;     // 2048 samples per CTA tile
 constexpr int DET_MAXW = 1 << (DEDISP_DETECT_MAX_WIDTHS - 1);
+constexpr int DET_SEGS = 8;                         // boxcar kernel: 256-sample segments per warp
+inline int det_own(int nwidths) { return 256 - ((((1 << (nwidths - 1)) - 1) + 7) & ~7); }   // positions a 256-sample warp segment owns
+static_assert(DET_MAXW <= 128, "a segment must own at least half of its samples");
 
 template <typename T>
 __global__ void __launch_bounds__(DET_THREADS) dedisp_detect_stats_kernel(const T *__restrict__ x, long long stride, long long n,
@@ -52,16 +56,24 @@ __global__ void __launch_bounds__(DET_THREADS) dedisp_detect_stats_kernel(const 
     }
 }
 
+// Boxcar + threshold. A warp owns a segment of 256 consecutive samples of one row, 8 per lane in registers;
+// the next width comes from the current one by y_2w[p] = y_w[p] + y_w[p + w], where p + w lives w/8 lanes
+// further (a shuffle) or, for w < 8, partly in the lane's own registers. Segments overlap by H = the largest
+// width rounded up to 8, so that every position a segment owns (the first 256 - H) finds all its windows
+// inside the segment. Because S/N is monotone in the window sum (rw > 0, every operation rounds
+// monotonically), "snr >= threshold" is "y >= Y_w" for the smallest representable Y_w that passes: thread k
+// finds Y_w for width 2^k once per CTA with the exact double expression, the scan compares in the row's
+// own type (one SETP per sample and width, OR-ed into one predicate per lane) and evaluates the double S/N
+// only for the rare hits, which one atomic counter compacts into the caller's list.
 template <typename T>
 __global__ void __launch_bounds__(DET_THREADS) dedisp_detect_boxcar_kernel(const T *__restrict__ x, long long stride, long long n, int nwidths,
                                                                              double threshold, const unsigned long long *__restrict__ stats,
                                                                              dedisp_candidate *__restrict__ cands, long long max_cands,
                                                                              unsigned long long *__restrict__ count) {
-    __shared__ T buf[2][DET_TILE + DET_MAXW];
     const int row_i = blockIdx.y;
     // mean and variance exactly as the definition orders them (explicitly rounded double operations)
     double mu, var;
-    if constexpr (sizeof(T) == 4 && !std::is_floating_point<T>::value) {
+    if constexpr (!std::is_floating_point<T>::value) {
         const long long s1 = (long long)stats[2 * row_i], s2 = (long long)stats[2 * row_i + 1];
         mu = __ddiv_rn((double)s1, (double)n);
         var = __dsub_rn(__ddiv_rn((double)s2, (double)n), __dmul_rn(mu, mu));
@@ -72,15 +84,6 @@ __global__ void __launch_bounds__(DET_THREADS) dedisp_detect_boxcar_kernel(const
     }
     if (!(var > 0.0)) return;
     const double sd = __dsqrt_rn(var);
-    const T *row = x + (size_t)row_i * stride;
-    const long long t0 = (long long)blockIdx.x * DET_TILE;
-    const int halo = (1 << (nwidths - 1)) - 1;
-    const int nload = (int)min((long long)DET_TILE + halo, n - t0);     // samples of the row available from t0
-    for (int i = threadIdx.x; i < DET_TILE + halo; i += DET_THREADS) buf[0][i] = i < nload ? row[t0 + i] : (T)0;
-    __syncthreads();
-    // snr is monotone in y (rw > 0, every operation rounds monotonically), so "snr >= threshold" is "y >= Y_w"
-    // for the smallest representable Y_w that passes: thread k finds Y_w for width 2^k once per CTA, the scan
-    // then compares in the row's own type and evaluates the double expression only for the rare candidates
     __shared__ T ycrit[DEDISP_DETECT_MAX_WIDTHS];
     __shared__ int ynone[DEDISP_DETECT_MAX_WIDTHS];
     if (threadIdx.x < nwidths) {
@@ -110,33 +113,73 @@ __global__ void __launch_bounds__(DET_THREADS) dedisp_detect_boxcar_kernel(const
         ynone[threadIdx.x] = none;
     }
     __syncthreads();
-    int cur = 0;
-    for (int k = 0, w = 1; k < nwidths; ++k, w *= 2) {
-        if (k > 0) {   // y_w[i] = y_{w/2}[i] + y_{w/2}[i + w/2], wherever the wider window still fits the loaded span
-            const int h = w / 2, lim = DET_TILE + halo - w + 1;
-            for (int i = threadIdx.x; i < lim; i += DET_THREADS) buf[cur ^ 1][i] = (T)(buf[cur][i] + buf[cur][i + h]);
-            cur ^= 1;
-            __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int H = ((1 << (nwidths - 1)) - 1 + 7) & ~7;              // overlap between neighbouring segments
+    const int own = 256 - H;                                       // positions a segment owns
+    const T *row = x + (size_t)row_i * stride;
+#pragma unroll 1
+    for (int rep = 0; rep < DET_SEGS; ++rep) {                     // DET_SEGS segments per warp: the critical values are found once per CTA
+    const long long t0 = (((long long)blockIdx.x * DET_SEGS + rep) * (DET_THREADS / 32) + (threadIdx.x >> 5)) * own;
+    if (t0 >= n) return;
+    T v[8];
+    const T *src = row + t0 + 8 * lane;
+    if (t0 + 256 <= n && (reinterpret_cast<uintptr_t>(src) & 15) == 0) {   // interior segment, 16-byte aligned: two vector loads
+        const uint4 a = __ldg(reinterpret_cast<const uint4 *>(src)), b = __ldg(reinterpret_cast<const uint4 *>(src) + 1);
+        const unsigned raw[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if constexpr (std::is_floating_point<T>::value) v[i] = __uint_as_float(raw[i]);
+            else v[i] = (T)raw[i];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { const long long t = t0 + 8 * lane + i; v[i] = t < n ? row[t] : (T)0; }
+    }
+#pragma unroll
+    for (int k = 0; k < DEDISP_DETECT_MAX_WIDTHS; ++k) {
+        if (k >= nwidths) break;
+        const int w = 1 << k;
+        if (k > 0) {                                               // y_w[p] = y_h[p] + y_h[p + h], h = w / 2
+            constexpr int KH = 1;
+            (void)KH;
+            const int h = w / 2;
+            T u[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                T partner;
+                if (h < 8) partner = i + h < 8 ? v[(i + h) & 7] : __shfl_down_sync(0xffffffffu, v[(i + h) & 7], 1);
+                else partner = __shfl_down_sync(0xffffffffu, v[i], h / 8);
+                u[i] = (T)(v[i] + partner);
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = u[i];
         }
         if (ynone[k]) continue;
         const T crit = ycrit[k];
-        for (int i = threadIdx.x; i < DET_TILE; i += DET_THREADS) {
-            if (t0 + i + w > n) break;                                  // the window must lie inside the row
-            const T y = buf[cur][i];
-            if (y >= crit) {
-                const double wm = __dmul_rn((double)w, mu);
-                const double rw = __ddiv_rn(1.0, __dmul_rn(sd, __dsqrt_rn((double)w)));
-                const double snr = __dmul_rn(__dsub_rn((double)y, wm), rw);
-                if (snr >= threshold) {                                // always true; kept as the definition's own test
-                    const unsigned long long slot = atomicAdd(count, 1ull);
-                    if ((long long)slot < max_cands) {
-                        dedisp_candidate c;
-                        c.dm_index = row_i; c.width = w; c.t = t0 + i; c.snr = snr;
-                        cands[slot] = c;
+        bool hit = false;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) hit |= v[i] >= crit;
+        if (hit) {
+            const double wm = __dmul_rn((double)w, mu);
+            const double rw = __ddiv_rn(1.0, __dmul_rn(sd, __dsqrt_rn((double)w)));
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int pos = 8 * lane + i;
+                const long long t = t0 + pos;
+                if (v[i] >= crit && pos < own && t + w <= n) {       // owned position, window inside the row
+                    const double snr = __dmul_rn(__dsub_rn((double)v[i], wm), rw);
+                    if (snr >= threshold) {                         // always true; kept as the definition's own test
+                        const unsigned long long slot = atomicAdd(count, 1ull);
+                        if ((long long)slot < max_cands) {
+                            dedisp_candidate c;
+                            c.dm_index = row_i; c.width = w; c.t = t; c.snr = snr;
+                            cands[slot] = c;
+                        }
                     }
                 }
             }
         }
+    }
     }
 }
 
@@ -155,7 +198,7 @@ int dedisp_detect(const void *d_block, int block_is_float, int ndm, long long ns
     unsigned long long *stats = count + 1;
     cudaError_t e = cudaMemsetAsync(d_work, 0, (size_t)ndm * 16 + 8, st);
     if (e != cudaSuccess) return DEDISP_ECUDA;
-    const dim3 g1((unsigned)((nsamp + DET_TILE * 8 - 1) / (DET_TILE * 8)), (unsigned)ndm), g2((unsigned)((nsamp + DET_TILE - 1) / DET_TILE), (unsigned)ndm);
+    const dim3 g1((unsigned)((nsamp + DET_TILE * 8 - 1) / (DET_TILE * 8)), (unsigned)ndm), g2((unsigned)((nsamp + (long long)det_own(nwidths) * (DET_THREADS / 32) * DET_SEGS - 1) / ((long long)det_own(nwidths) * (DET_THREADS / 32) * DET_SEGS)), (unsigned)ndm);
     if (block_is_float) {
         dedisp_detect_stats_kernel<float><<<g1, DET_THREADS, 0, st>>>((const float *)d_block, stride, nsamp, stats);
         dedisp_detect_boxcar_kernel<float><<<g2, DET_THREADS, 0, st>>>((const float *)d_block, stride, nsamp, nwidths, threshold, stats, d_cands, max_cands, count);
