@@ -54,9 +54,11 @@ enum dedisp_kernel {
 enum dedisp_plan_flags {
     DEDISP_PLAN_DEFAULT = 0,
     DEDISP_PLAN_HOST_ONLY = 1, /* build host tables only; no CUDA call is made; execute -> EUNSUPPORTED */
-    DEDISP_PLAN_TIME_MAJOR = 2 /* the plan will be fed TIME-major packed input through dedisp_execute_time_major:
+    DEDISP_PLAN_TIME_MAJOR = 2, /* the plan will be fed TIME-major packed input through dedisp_execute_time_major:
                                   in_dtype must be DEDISP_U8 and nchans a multiple of 16 (else EINVAL); sub-bands
                                   are cut at multiples of 16 channels. Channel-major calls stay available. */
+    DEDISP_PLAN_NO_PACKED = 4  /* DEDISP_U8 plans: sum in fp32 like the other dtypes instead of as packed 16-bit
+                                  pairs on the integer pipes (same results bit for bit; kept for comparison) */
 };
 
 /* ---- subsystem (2): shift-table builder ("the shifting value

@@ -20,6 +20,7 @@ U8, F16, F32 = 0, 1, 2
 KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND = 0, 1, 2, 3
 PLAN_HOST_ONLY = 1
 PLAN_TIME_MAJOR = 2
+PLAN_NO_PACKED = 4
 
 DTYPE_CODE = {"u8": U8, "f16": F16, "f32": F32}
 _TORCH_IN = {U8: torch.uint8, F16: torch.float16, F32: torch.float32}
@@ -116,11 +117,11 @@ def _stream_ptr(stream) -> int:
 class Plan:
     """``dedisp_plan``: shift table + kernel metadata for one (band, sampling, DM list, dtype)."""
 
-    def __init__(self, nchans, fch1, foff, tsamp, dm_list, dtype, host_only: bool = False, time_major: bool = False):
+    def __init__(self, nchans, fch1, foff, tsamp, dm_list, dtype, host_only: bool = False, time_major: bool = False, packed: bool = True):
         self._h = ctypes.c_void_p()
         self.dtype = DTYPE_CODE[dtype] if isinstance(dtype, str) else int(dtype)
         dm, dmp = _dm(dm_list)
-        flags = (PLAN_HOST_ONLY if host_only else 0) | (PLAN_TIME_MAJOR if time_major else 0)
+        flags = (PLAN_HOST_ONLY if host_only else 0) | (PLAN_TIME_MAJOR if time_major else 0) | (0 if packed else PLAN_NO_PACKED)
         rc = lib().dedisp_plan_create_ex(ctypes.byref(self._h), int(nchans), float(fch1), float(foff), float(tsamp),
                                          dmp, dm.size, self.dtype, flags)
         if rc:
@@ -130,8 +131,8 @@ class Plan:
         self.max_shift = int(lib().dedisp_plan_max_shift(self._h))
 
     @classmethod
-    def from_config(cls, cfg, host_only: bool = False, time_major: bool = False) -> "Plan":
-        return cls(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), cfg.dtype, host_only, time_major)
+    def from_config(cls, cfg, host_only: bool = False, time_major: bool = False, packed: bool = True) -> "Plan":
+        return cls(cfg.nchans, cfg.fch1, cfg.foff, cfg.tsamp, cfg.dm_list(), cfg.dtype, host_only, time_major, packed)
 
     def _check(self, rc, what):
         if rc:

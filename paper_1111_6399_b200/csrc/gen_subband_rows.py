@@ -134,7 +134,94 @@ def generate(D, K, S, G, rec_stride):
     return head + params + ("asm volatile(\n%s\n    : %s\n    : \"r\"(rp0), \"r\"(slot0), \"r\"(slot_bytes), \"r\"(nch)\n    : \"memory\");\n#endif\n" % (text, outs))
 
 
+def generate_i16(D, K, OMAX, rec_stride):
+    """The same stage loop for u8 plans that sum PACKED 16-bit pairs on the integer pipes (``subband_rows_i16.inc``).
+
+    A 32-bit word holds two consecutive samples (the earlier one in the low half), a thread owns D rows x K
+    words = 2K samples, and a row's in-window offset o (in SAMPLES, 0..OMAX) splits into a word offset o >> 1
+    and a half-word bit: even offsets are K ``add.u32`` on whole words, odd ones K funnel-shift + add pairs that
+    ptxas fuses into one ``LEA.HI`` each (acc + ((x[k+1] << 16) | (x[k] >> 16))).  No lane ever carries
+    into its neighbour because a pass sums at most 257 channels of values <= 255 (plan.h SB16_CHMAX).
+    Word offsets cost nothing here (no 64-bit register pairing), so every ROW jumps on its own offset: D
+    jumps per channel and (OMAX + 1) bodies per row, for twice the samples of the fp32 loop.
+    Operands: %0.. acc[j][k2] (b64 = two words = four samples, "+l"), then rp0, slot0, slot_bytes, nch as
+    above; a record is {lo: one offset per row, 8 bits each, row 0 lowest; hi: window base in 8-byte pairs}."""
+    assert K % 2 == 0 and OMAX + 1 <= 255
+    K2 = K // 2
+    NP = ((OMAX >> 1) + K + 1 + 1) // 2               # 8-byte pairs a thread loads per channel
+    NA = D * K2
+    RP0, SLOT0, SLOTB, NCH = ("%%%d" % (NA + i) for i in range(4))
+    EXIT = OMAX + 1
+    L = ["{", ".reg .b32 a<%d>, x<%d>, f<%d>;" % (D * K, 2 * NP, K),
+         ".reg .b32 t<%d>, rlo, rhi, nlo, nhi, cnt, sa, rp, sl;" % D, ".reg .pred pm;"]
+    for g in range(D):
+        tgt = ["B%d_%d" % (g, o) for o in range(OMAX + 1)] + (["DONE"] if g == 0 else [])
+        L.append("TP%d: .branchtargets %s;" % (g, ", ".join(tgt)))
+    for i in range(NA):
+        L.append("mov.b64 {a%d, a%d}, %%%d;" % (2 * i, 2 * i + 1, i))
+
+    def ids(src):
+        return ["and.b32 t0, %s, 255;" % src if g == 0 else "bfe.u32 t%d, %s, %d, 8;" % (g, src, 8 * g) for g in range(D)]
+
+    def load(m, pred):
+        return "%sld.shared.v2.b32 {x%d, x%d}, [sa+%d];" % ("@pm " if pred else "", 2 * m, 2 * m + 1, 8 * m)
+
+    L += ["mov.u32 rp, %s;" % RP0, "mov.u32 sl, %s;" % SLOT0, "mov.u32 cnt, %s;" % NCH,
+          "ld.shared.v2.u32 {rlo, rhi}, [rp];", "shl.b32 sa, rhi, 3;", "add.u32 sa, sa, sl;"]
+    L += [load(m, False) for m in range(NP)]
+    L += ["add.u32 rp, rp, %d;" % rec_stride, "add.u32 sl, sl, %s;" % SLOTB, "ld.shared.v2.u32 {nlo, nhi}, [rp];"]
+    L += ids("rlo")
+    L.append("brx.idx.uni t0, TP0;")
+
+    def rows(j, o, prefetch):
+        ow, ob = o >> 1, o & 1
+        out = []
+        if prefetch:                                    # pairs this row never reaches from below
+            out += [load(m, True) for m in range(NP) if 2 * m + 1 < ow]
+        for k in range(K):
+            acc = "a%d" % (j * K + k)
+            if ob:
+                out += ["shf.r.wrap.b32 f%d, x%d, x%d, 16;" % (k, k + ow, k + ow + 1), "add.u32 %s, %s, f%d;" % (acc, acc, k)]
+            else:
+                out.append("add.u32 %s, %s, x%d;" % (acc, acc, k + ow))
+            if prefetch and (k + ow) & 1:
+                out.append(load((k + ow) >> 1, True))  # both words of this pair have been read for the last time
+        if prefetch:                                    # the pair the last add straddles or stops in, and those above
+            done = {m for m in range(NP) if 2 * m + 1 < ow} | {(k + ow) >> 1 for k in range(K) if (k + ow) & 1}
+            out += [load(m, True) for m in range(NP) if m not in done]
+        return out
+
+    for g in range(D):
+        last = g == D - 1
+        for o in range(OMAX + 1):
+            L.append("B%d_%d:" % (g, o))
+            if not last:
+                L += rows(g, o, False)
+                L.append("brx.idx.uni t%d, TP%d;" % (g + 1, g + 1))
+                continue
+            L += ["add.u32 cnt, cnt, -1;", "setp.ne.u32 pm, cnt, 0;", "shl.b32 sa, nhi, 3;", "add.u32 sa, sa, sl;"]
+            L += rows(g, o, True)
+            L += ids("nlo")
+            L += ["@!pm mov.u32 t0, %d;" % EXIT, "add.u32 rp, rp, %d;" % rec_stride, "add.u32 sl, sl, %s;" % SLOTB,
+                  "ld.shared.v2.u32 {nlo, nhi}, [rp];", "brx.idx.uni t0, TP0;"]
+    L.append("DONE:")
+    for i in range(NA):
+        L.append("mov.b64 %%%d, {a%d, a%d};" % (i, 2 * i, 2 * i + 1))
+    L.append("}")
+    text = "\n".join('    "%s\\n"' % x for x in L)
+    outs = ", ".join('"+l"(acc[%d][%d])' % (j, k) for j in range(D) for k in range(K2))
+    head = ("// GENERATED by gen_subband_rows.py (generate_i16 %d %d %d %d) - do not edit.\n"
+            "// One pipeline stage of the SUBBAND kernel for packed 16-bit sums: per channel %d LDS.64 and one jump per row on its\n"
+            "// own offset into %d bodies; the last row's bodies prefetch the next channel's window and jump straight into it.\n"
+            % (D, K, OMAX, rec_stride, NP, OMAX + 1))
+    params = ("#ifdef SB_ROWS_PARAMS\n"
+              "static_assert(SB_D == %d && SB_K == %d && SB16_OMAX == %d && SB_REC_STRIDE == %d && SB_WPAIRS == %d, \"regenerate subband_rows_i16.inc (gen_subband_rows.py)\");\n"
+              "#else\n" % (D, K, OMAX, rec_stride, NP))
+    return head + params + ("asm volatile(\n%s\n    : %s\n    : \"r\"(rp0), \"r\"(slot0), \"r\"(slot_bytes), \"r\"(nch)\n    : \"memory\");\n#endif\n" % (text, outs))
+
+
 DEFAULT = (4, 26, 5, 2, 96)
+DEFAULT_I16 = (4, 26, 11, 96)
 
 if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]
@@ -143,3 +230,7 @@ if __name__ == "__main__":
     with open(path, "w") as f:
         f.write(generate(*a))
     print(path, *a)
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "subband_rows_i16.inc")
+    with open(path, "w") as f:
+        f.write(generate_i16(a[0], a[1], DEFAULT_I16[2], a[4]))
+    print(path, a[0], a[1], DEFAULT_I16[2], a[4])

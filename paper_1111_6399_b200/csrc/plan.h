@@ -59,6 +59,17 @@ constexpr int SB_EP_WORDS = SB_T + 8;     // epilogue transpose buffer of one wa
 // staged 16-byte chunks per channel the slot can hold, a multiple of 32
 constexpr int SB_NCH_MAX = ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 * 32;
 
+// Packed 16-bit variant for u8 plans (subband_rows_i16.inc): a 32-bit word holds TWO samples, so the same
+// thread tile of SB_K words covers 2*SB_K samples per row, and the sums run on the integer pipes
+// (profiles/r2_microbench.md, packed_add.cu). Offsets are in samples; window bases stay 8 bytes = 4 samples apart.
+constexpr int SB16_KS = 2 * SB_K;         // samples per thread and row
+constexpr int SB16_T = 32 * SB16_KS;      // u-samples per CTA tile
+constexpr int SB16_OMAX = 11;             // largest in-window offset: word offset 5 + the half-word bit
+constexpr int SB16_S = SB16_OMAX - 3;     // spread bound of a thread's rows (the smallest offset is 0..3)
+constexpr int SB16_CHMAX = 257;           // channels per pass: 257 * 255 = 65535 still fits a 16-bit lane
+constexpr int SB16_EP_WORDS = SB16_T + 8;
+static_assert((SB16_OMAX >> 1) + SB_K + 1 <= 2 * SB_WPAIRS, "the packed window must fit the SB_WPAIRS pairs a thread loads");
+
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;
     int max_skew = 0;                 // max over the pass's DM rows of s(c_ref, d)
@@ -88,14 +99,16 @@ struct SbRun {
 
 struct SubbandGeom {
     bool ok = false;
+    bool i16 = false;                 // u8 plan summed as packed 16-bit pairs (units below in samples all the same)
+    int tile_t = SB_T;                // u-samples per CTA tile (SB_T or SB16_T)
     std::vector<SubbandPass> passes;  // launch order: the k-th sub-band of every DM range, k = 0, 1, ...
     std::vector<int> launch_begin;    // [nlaunch + 1]: ordered launch g runs passes [launch_begin[g], launch_begin[g + 1])
     int ngroups = 0, nblk = 0;
     int nranges = 0;                  // DM-block ranges, each with its own sub-band partition (1 for uniform DM plans)
     // [nblk][nchans][SB_WARPS] per (block, channel, group): low word = joint pattern ids, 8 bits per dispatch group (group 0 lowest):
-    // (o_a*(S+2) + o_b)..., high word = window base a in 8-byte pairs (subband.cu)
+    // (o_a*(S+2) + o_b)... (i16: one offset per row, 8 bits each, row 0 lowest), high word = window base a in 8-byte pairs (subband.cu)
     std::vector<uint64_t> records;
-    // per (block, channel): {window base r (multiple of 4, relative to u), chunks to stage}
+    // per (block, channel): {window base r (multiple of 4 samples, i16: 8; relative to u), 16-byte chunks to stage}
     std::vector<int32_t> meta;        // [nblk][nchans][2]
     std::vector<int32_t> skew;        // [npasses][ndm] = s(c_ref(pass), d)
     uint64_t *d_records = nullptr;

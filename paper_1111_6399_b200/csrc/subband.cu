@@ -32,13 +32,30 @@
 
 namespace {
 
-inline int floor4(int v) { return v & ~3; }  // toward -inf, two's complement
+// Units of the window geometry. fp32 ring: a word is one sample. Packed 16-bit ring (u8 plans, SubbandGeom::i16):
+// a word is two samples; everything below is in SAMPLES.
+struct SbUnits {
+    int aunit;      // samples per 8-byte window-base step
+    int rb_align;   // the staged window starts at a multiple of this (one 16-byte chunk)
+    int omax, spread;
+    int ks;         // samples per thread and row
+    int ws;         // samples in the window a thread loads (SB_WPAIRS pairs)
+    int cs;         // samples per 16-byte chunk
+    int chmax;      // channels per pass
+    bool joint;     // record holds joint pattern ids per SB_G rows (fp32) / one offset per row (i16)
+};
+inline SbUnits sb_units(bool i16) {
+    return i16 ? SbUnits{4, 8, SB16_OMAX, SB16_S, SB16_KS, 4 * SB_WPAIRS, 8, SB16_CHMAX, false}
+               : SbUnits{2, 4, SB_OMAX, SB_S, SB_K, 2 * SB_WPAIRS, 4, INT32_MAX, true};
+}
 
 // Residual-delay geometry of channels [cb, ce) against reference channel cr. Returns false if some
 // group's in-window offsets would exceed SB_OMAX or a block's staged window exceeds SB_NCH_MAX.
 // With `emit`, writes records/meta for those channels.
 bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, int b1) {
     const int ndm = p->ndm, ngroups = p->sb.ngroups, nblk = p->sb.nblk;
+    const SbUnits U = sb_units(p->sb.i16);
+    if (ce - cb > U.chmax) return false;
     const int32_t *sref = p->shifts.data() + (size_t)cr * ndm;
     const int gslots = nblk * SB_WARPS;
     std::vector<int> gmin(gslots), gmax(gslots);
@@ -59,16 +76,16 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
         for (int b = b0; b < b1; ++b) {
             int bmin = INT32_MAX;
             for (int w = 0; w < SB_WARPS; ++w) bmin = std::min(bmin, gmin[b * SB_WARPS + w]);
-            const int rbase = floor4(bmin);
+            const int rbase = bmin & ~(U.rb_align - 1);  // toward -inf, two's complement
             // window base of a group inside the block's staged region in 8-byte pairs; what is left of
             // the residual delays are the in-window offsets
-            constexpr int AUNIT = 2;
+            const int AUNIT = U.aunit;
             int amax = 0;
             for (int w = 0; w < SB_WARPS; ++w) {
                 const int q = b * SB_WARPS + w;
                 const int a = (gmin[q] - rbase) / AUNIT;
-                if (gmax[q] - rbase - AUNIT * a > SB_OMAX) return false;
-                if (gmax[q] - gmin[q] > SB_S) return false;
+                if (gmax[q] - rbase - AUNIT * a > U.omax) return false;
+                if (gmax[q] - gmin[q] > U.spread) return false;
                 amax = std::max(amax, a);
                 if (emit) {
                     uint64_t rec = (uint64_t)a << 32;
@@ -77,6 +94,7 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
                     for (int j = 0; j < SB_D; ++j) {
                         const int d = std::min(qq * SB_D + j, ndm - 1);
                         const int o = (sc[d] - sref[d]) - rbase - AUNIT * a;
+                        if (!U.joint) { lo |= (uint32_t)o << (8 * j); continue; }   // one offset per row
                         // 8 bits per dispatch group: pattern id, the group's first row most significant
                         const int g = j / SB_G, sh = 8 * g;
                         const uint32_t id = ((lo >> sh) & 255u) * (SB_S + 2) + (uint32_t)o;
@@ -86,7 +104,7 @@ bool pass_geometry(dedisp_plan *p, int cb, int ce, int cr, bool emit, int b0, in
                 }
             }
             // staged 16-byte chunks: the furthest lane of the furthest group must find its whole window
-            const int nch = (2 * amax + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
+            const int nch = (AUNIT * amax + U.ks * 31 + U.ws + U.cs - 1) / U.cs;
             if (nch > SB_NCH_MAX || amax > 0xffff) return false;
             if (emit) {
                 p->sb.meta[((size_t)b * p->nchans + c) * 2 + 0] = rbase;
@@ -122,22 +140,24 @@ int pick_ref(const dedisp_plan *p, int cb, int ce) {
 
 // raw path: bytes per raw channel slot (window bytes + up to 15 lead bytes, rounded up to 16, + one
 // spare chunk the realigning loads may touch)
-static int sb_raw_slot_bytes(int slot_chunks, int esize) { return ((slot_chunks * 4 * esize + 15 + 15) & ~15) + 16; }
+static int sb_raw_slot_bytes(int slot_chunks, int esize, int cs) { return ((slot_chunks * cs * esize + 15 + 15) & ~15) + 16; }
 
 // dynamic shared memory of the SUBBAND kernel for `cb` channels per stage (esize > 0: raw path)
-static size_t sb_smem_bytes(int cb, int slot_chunks, int esize) {
+static size_t sb_smem_bytes(int cb, int slot_chunks, int esize, bool i16) {
     size_t b = (size_t)SB_STAGES * cb * slot_chunks * 16 + (size_t)(SB_STAGES * cb + 1) * SB_REC_STRIDE + 16 * SB_STAGES + 16;
     b = (b + 15) / 16 * 16;
-    b += (size_t)SB_WARPS * SB_EP_WORDS * sizeof(float);
-    if (esize > 0) b += (size_t)cb * sb_raw_slot_bytes(slot_chunks, esize);
+    b += (size_t)SB_WARPS * (i16 ? SB16_EP_WORDS : SB_EP_WORDS) * sizeof(float);
+    if (esize > 0) b += (size_t)cb * sb_raw_slot_bytes(slot_chunks, esize, sb_units(i16).cs);
     return b;
 }
 
 
-void subband_build(dedisp_plan *p) {
+static void subband_build_as(dedisp_plan *p, const bool i16) {
     p->sb = SubbandGeom();
     SubbandGeom &sb = p->sb;
     const int nchans = p->nchans, ndm = p->ndm;
+    sb.i16 = i16;
+    sb.tile_t = i16 ? SB16_T : SB_T;
     sb.ngroups = (ndm + SB_D - 1) / SB_D;
     sb.nblk = (sb.ngroups + SB_WARPS - 1) / SB_WARPS;
     const size_t gslots = (size_t)sb.nblk * SB_WARPS;
@@ -245,16 +265,26 @@ void subband_build(dedisp_plan *p) {
     // as many channels per stage as fit the 227 KB a CTA may opt into (fewer, longer stages: fewer hand-overs)
     sb.slot_chunks = sb.max_nch + 1;
     const int esize = dtype_esize(p->dtype);
-    sb.raw_slot_bytes = sb_raw_slot_bytes(sb.slot_chunks, esize);
+    sb.raw_slot_bytes = sb_raw_slot_bytes(sb.slot_chunks, esize, sb_units(i16).cs);
     auto pick = [&](int es, int &cb_out, size_t &smem_out) {
         cb_out = SB_CB;
         for (int cb = SB_CB_MAX; cb > SB_CB; --cb)
-            if (sb_smem_bytes(cb, sb.slot_chunks, es) <= 227u * 1024u) { cb_out = cb; break; }
-        smem_out = sb_smem_bytes(cb_out, sb.slot_chunks, es);
+            if (sb_smem_bytes(cb, sb.slot_chunks, es, i16) <= 227u * 1024u) { cb_out = cb; break; }
+        smem_out = sb_smem_bytes(cb_out, sb.slot_chunks, es, i16);
     };
     pick(0, sb.cb, sb.smem);
     pick(esize, sb.cb_raw, sb.smem_raw);
     sb.ok = true;
+}
+
+void subband_build(dedisp_plan *p) {
+    // u8 plans sum packed 16-bit pairs on the integer pipes (time-major plans keep the fp32 ring their
+    // scatter writes); should that geometry not be admitted, the fp32 one is tried
+    if (p->dtype == DEDISP_U8 && !p->time_major && !(p->flags & DEDISP_PLAN_NO_PACKED)) {
+        subband_build_as(p, true);
+        if (p->sb.ok) return;
+    }
+    subband_build_as(p, false);
 }
 
 // Rebuild s(c,d) from the packed records (+ meta + skew) and compare with the table: the records
@@ -264,25 +294,31 @@ long long subband_verify_records(const dedisp_plan *p) {
     const SubbandGeom &sb = p->sb;
     if (!sb.ok) return -1;
     const int ndm = p->ndm;
-    const size_t gslots = (size_t)sb.nblk * SB_WARPS;
+    const SbUnits U = sb_units(sb.i16);
     long long bad = 0;
     std::vector<int> seen(p->nchans, 0);   // DM blocks that cover channel c: every channel exactly once per block
     for (size_t g = 0; g < sb.passes.size(); ++g) {
         const SubbandPass &ps = sb.passes[g];
         for (int c = ps.c_begin; c < ps.c_end; ++c) {
             seen[c] += ps.blk_end - ps.blk_begin;
+            if (ps.c_end - ps.c_begin > U.chmax) ++bad;
             for (int d = ps.blk_begin * SB_ROWS; d < std::min(ndm, ps.blk_end * SB_ROWS); ++d) {
                 const int q = d / SB_D, j = d % SB_D, b = q / SB_WARPS;
                 const uint64_t rec = sb.records[((size_t)b * p->nchans + c) * SB_WARPS + q % SB_WARPS];
                 const int a = (int)((rec >> 32) & 0xffff);
-                uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
-                for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
-                const int o = (int)(id % (SB_S + 2));
+                int o;
+                if (U.joint) {
+                    uint32_t id = ((uint32_t)rec >> (8 * (j / SB_G))) & 255u;
+                    for (int jj = SB_G - 1; jj > j % SB_G; --jj) id /= (SB_S + 2);
+                    o = (int)(id % (SB_S + 2));
+                } else {
+                    o = (int)(((uint32_t)rec >> (8 * j)) & 255u);
+                }
                 const int rbase = sb.meta[((size_t)b * p->nchans + c) * 2];
                 const int nch = sb.meta[((size_t)b * p->nchans + c) * 2 + 1];
-                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + 2 * a + o;
-                const int need = (2 * a + SB_K * 31 + 2 * SB_WPAIRS + 3) / 4;
-                if (s != p->shifts[(size_t)c * ndm + d] || need > nch || (rbase & 3) || o > SB_OMAX) ++bad;
+                const long long s = (long long)sb.skew[g * (size_t)ndm + d] + rbase + U.aunit * a + o;
+                const int need = (U.aunit * a + U.ks * 31 + U.ws + U.cs - 1) / U.cs;
+                if (s != p->shifts[(size_t)c * ndm + d] || need > nch || (rbase & (U.rb_align - 1)) || o > U.omax) ++bad;
             }
         }
     }
@@ -322,6 +358,7 @@ static_assert(SB_NCH_MAX % 32 == 0, "staging loop");
 static_assert(SB_K % 2 == 0 && (SB_K / 2) % 2 == 1, "K/2 odd: LDS.64 conflict-free in the plain layout");
 #define SB_ROWS_PARAMS
 #include "subband_rows.inc"
+#include "subband_rows_i16.inc"
 #undef SB_ROWS_PARAMS
 
 __device__ __forceinline__ void sb_cp_async16_zs(unsigned sa, const void *gmem, int src_bytes) {
@@ -395,13 +432,14 @@ struct SbTile {
     const int32_t *skew;
 };
 
+template <int TT>   // u-samples per tile
 __device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
     const int grid = (int)gridDim.x;
     for (;;) {
         if (t.p >= A.pass_hi) return false;
         const SbPassDev P = A.passes[t.p];
         const int b0 = max(A.blk_lo, P.blk_begin), nb = min(A.blk_hi, P.blk_end) - b0;
-        const int ntu = (int)((A.nsamp_out + P.max_skew + SB_T - 1) / SB_T);
+        const int ntu = (int)((A.nsamp_out + P.max_skew + TT - 1) / TT);
         const int ntiles = nb > 0 ? A.nbeams * ntu * nb : 0;
         if (t.w < 0) t.w = ((int)blockIdx.x + grid - t.rot) % grid;
         if (t.w >= ntiles) { t.rot = (t.rot + ntiles % grid) % grid; ++t.p; t.w = -1; continue; }
@@ -410,11 +448,11 @@ __device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
         t.blk = b0 + w % nb;
         const int rest = w / nb;
         t.beam = rest / ntu;
-        t.U0 = (long long)(rest % ntu) * SB_T;
+        t.U0 = (long long)(rest % ntu) * TT;
         t.skew = A.skew + (size_t)t.p * A.ndm;
         const int d_first = t.blk * SB_ROWS, d_last = min(A.ndm, d_first + SB_ROWS) - 1;
         // rows of this block are valid for u in [skew(d), skew(d) + nsamp_out)
-        if (t.U0 + SB_T <= (long long)__ldg(t.skew + d_first) || t.U0 >= (long long)__ldg(t.skew + d_last) + A.nsamp_out) continue;
+        if (t.U0 + TT <= (long long)__ldg(t.skew + d_first) || t.U0 >= (long long)__ldg(t.skew + d_last) + A.nsamp_out) continue;
         t.c_begin = P.c_begin;
         t.c_end = P.c_end;
         t.first = P.first;
@@ -439,6 +477,15 @@ __device__ __forceinline__ float4 sb_raw4(unsigned raw_u32, unsigned off) {
         return make_float4(__uint_as_float(lds(wa)), __uint_as_float(lds(wa + 4)), __uint_as_float(lds(wa + 8)), __uint_as_float(lds(wa + 12)));
     }
 }
+// eight u8 samples of a raw staged window at byte offset `off` as four words of packed 16-bit pairs
+// (earlier sample in the low half)
+__device__ __forceinline__ uint4 sb_raw8_u16(unsigned raw_u32, unsigned off) {
+    const unsigned wa = raw_u32 + (off & ~3u), sh = (off & 3u) * 8u;
+    auto lds = [](unsigned a) { unsigned v; asm volatile("ld.shared.b32 %0, [%1];\n" : "=r"(v) : "r"(a)); return v; };
+    const unsigned w0 = lds(wa), w1 = lds(wa + 4), w2 = lds(wa + 8);
+    const unsigned a = __funnelshift_r(w0, w1, sh), b = __funnelshift_r(w1, w2, sh);
+    return make_uint4(__byte_perm(a, 0, 0x4140), __byte_perm(a, 0, 0x4342), __byte_perm(b, 0, 0x4140), __byte_perm(b, 0, 0x4342));
+}
 template <typename TIN> __device__ __forceinline__ float sb_to_f32(TIN v) { return (float)v; }
 template <> __device__ __forceinline__ float sb_to_f32<__half>(__half v) { return __half2float(v); }
 
@@ -458,7 +505,12 @@ template <> __device__ __forceinline__ float sb_to_f32<__half>(__half v) { retur
 // channel windows of the ring: the corner turn costs no extra pass over the input and no staging buffer.
 template <typename TIN, int MODE>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
-    constexpr bool RAW = MODE == 1;
+    constexpr bool I16 = MODE == 6;   // u8 plan summed as packed 16-bit pairs: ring words hold two samples
+    constexpr bool RAW = MODE == 1 || I16;
+    constexpr int TT = I16 ? SB16_T : SB_T;                  // u-samples per tile
+    constexpr int CS = I16 ? 8 : 4;                          // samples per staged 16-byte chunk
+    constexpr int EPW = I16 ? SB16_EP_WORDS : SB_EP_WORDS;   // words of a warp's transpose buffer
+    static_assert(!I16 || std::is_same<TIN, uint8_t>::value, "packed sums are for u8 input");
     constexpr int TMB = MODE == 2 ? 8 : MODE == 3 ? 4 : MODE == 4 ? 2 : MODE == 5 ? 1 : 0;   // time-major: bits per sample
     constexpr bool CONV = RAW || TMB != 0;                                                   // producer warps write the ring
     extern __shared__ __align__(16) unsigned char sb_smem[];
@@ -474,7 +526,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     const unsigned bar_empty = bar_full + 8u * SB_STAGES;
     const unsigned bar_raw_full = bar_empty + 8u * SB_STAGES, bar_raw_empty = bar_raw_full + 8u;
     const unsigned ep_off = (bar_raw_empty + 8u - sdata_base + 15u) & ~15u;
-    const unsigned raw_base = sdata_base + ep_off + SB_WARPS * SB_EP_WORDS * 4;
+    const unsigned raw_base = sdata_base + ep_off + SB_WARPS * EPW * 4;
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < SB_STAGES; ++b) { sb_mbar_init(bar_full + 8u * b, CONV ? 4 : 32); sb_mbar_init(bar_empty + 8u * b, SB_WARPS); }
@@ -492,7 +544,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         if constexpr (TMB != 0) {
             const int pw = warp - SB_WARPS;
             const unsigned char *inb = reinterpret_cast<const unsigned char *>(A.in);
-            while (sb_next_tile(A, t)) {
+            while (sb_next_tile<TT>(A, t)) {
                 const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
                 for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {   // CB == 16, c0 % 16 == 0 (plan built with DEDISP_PLAN_TIME_MAJOR)
                     const int buf = it % SB_STAGES, k = it / SB_STAGES;
@@ -560,7 +612,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             const int pw = warp - SB_WARPS;
             constexpr long long ES = (long long)sizeof(TIN);
             const long long in_bytes = A.in_total * ES;
-            while (sb_next_tile(A, t)) {
+            while (sb_next_tile<TT>(A, t)) {
                 const char *inb = reinterpret_cast<const char *>(A.in) + (size_t)t.beam * A.in_beam * ES;
                 const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
                 for (int c0 = t.c_begin; c0 < t.c_end; c0 += CB, ++it) {
@@ -575,7 +627,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                         nch = mt.y;
                         g = ((long long)c * A.in_stride + t.U0 + mt.x) * ES;
                         lead = (unsigned)((reinterpret_cast<uintptr_t>(inb) + (unsigned long long)g) & 15u);
-                        rb = (lead + 4u * (unsigned)mt.y * (unsigned)ES + 15u) & ~15u;
+                        rb = (lead + (unsigned)CS * (unsigned)mt.y * (unsigned)ES + 15u) & ~15u;
                         return g - lead >= 0 && g - lead + rb <= in_bytes;
                     };
                     if (pw == 0) {   // copy warp: lane l copies the raw window of channel c0 + l with one TMA bulk copy
@@ -600,7 +652,27 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                         long long g; unsigned lead, rb; int nch;
                         const bool interior = window(c0 + cc, g, lead, rb, nch);
                         const unsigned dst = sdata_base + buf * stage_bytes + cc * slot_bytes;
-                        if (interior) {
+                        if constexpr (I16) {
+                            if (interior) {
+                                const unsigned raw = raw_base + cc * (unsigned)A.raw_slot_bytes;
+                                for (int i = lane; i < nch; i += 32) {
+                                    const uint4 v = sb_raw8_u16(raw, lead + 8u * i);
+                                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};\n" ::"r"(dst + 16u * i), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                                }
+                            } else {
+                                const uint8_t *src = reinterpret_cast<const uint8_t *>(inb);
+                                for (int i = lane; i < nch; i += 32) {
+                                    unsigned v[4];
+#pragma unroll
+                                    for (int q = 0; q < 4; ++q) {
+                                        const long long e = g + 8 * i + 2 * q;
+                                        const unsigned lo = e >= 0 && e < A.in_total ? src[e] : 0u, hi = e + 1 >= 0 && e + 1 < A.in_total ? src[e + 1] : 0u;
+                                        v[q] = lo | (hi << 16);
+                                    }
+                                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};\n" ::"r"(dst + 16u * i), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+                                }
+                            }
+                        } else if (interior) {
                             const unsigned raw = raw_base + cc * (unsigned)A.raw_slot_bytes;
                             for (int i = lane; i < nch; i += 32) {
                                 const float4 v = sb_raw4<TIN>(raw, lead + 4u * (unsigned)ES * i);
@@ -627,7 +699,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             return;
         }
         if (warp != SB_WARPS) return;
-        while (sb_next_tile(A, t)) {
+        while (sb_next_tile<TT>(A, t)) {
             const float *in = reinterpret_cast<const float *>(A.in) + (size_t)t.beam * A.in_beam;
             const int2 *meta = A.meta + (size_t)t.blk * A.nchans;
             const uint64_t *recs = A.records + (size_t)t.blk * A.nchans * SB_WARPS;
@@ -675,8 +747,8 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
     // ---------------- consumer warps
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(SbRegs<CONV>::consumer));
     const unsigned sdata_u32 = sdata_base + 4u * SB_K * lane;
-    float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * SB_EP_WORDS;
-    while (sb_next_tile(A, t)) {
+    float *ep = reinterpret_cast<float *>(sb_smem + ep_off) + (size_t)warp * EPW;
+    while (sb_next_tile<TT>(A, t)) {
         sb_u64 acc[SB_D][SB_K / 2];
 #pragma unroll
         for (int j = 0; j < SB_D; ++j)
@@ -690,7 +762,11 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             // the stage's channels, threaded: records are warp-uniform {x = pattern ids, y = window base in pairs}
             const unsigned rp0 = srec_base + (buf * CB * SB_WARPS + warp) * 8u;
             const unsigned slot0 = sdata_u32 + buf * stage_bytes;
+            if constexpr (I16) {
+#include "subband_rows_i16.inc"
+            } else {
 #include "subband_rows.inc"
+            }
             __syncwarp();
             if (lane == 0) sb_mbar_arrive(bar_empty + 8u * buf);
         }
@@ -712,8 +788,25 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             float *orow = out + (size_t)d * A.out_stride;
             const int sh = A.out_vec4 ? (int)(t0 & 3) : 0;                 // word 4g of the buffer <-> t = t0 - sh + 4g
             __syncwarp();
-            const unsigned wbase = ep_u32 + 4u * (unsigned)(SB_K * lane + sh);
-            if (!(sh & 1)) {
+            const unsigned wbase = ep_u32 + 4u * (unsigned)((I16 ? SB16_KS : SB_K) * lane + sh);
+            if constexpr (I16) {
+                // a 64-bit accumulator = four samples as 16-bit integers; as fp32: 0x4B00hhhh is 2^23 + h exactly
+#pragma unroll
+                for (int k2 = 0; k2 < SB_K / 2; ++k2) {
+                    const unsigned lo = (unsigned)acc[j][k2], hi = (unsigned)(acc[j][k2] >> 32);
+                    const float f0 = __uint_as_float(__byte_perm(lo, 0x4B000000u, 0x7610)) - 8388608.f, f1 = __uint_as_float(__byte_perm(lo, 0x4B000000u, 0x7632)) - 8388608.f;
+                    const float f2 = __uint_as_float(__byte_perm(hi, 0x4B000000u, 0x7610)) - 8388608.f, f3 = __uint_as_float(__byte_perm(hi, 0x4B000000u, 0x7632)) - 8388608.f;
+                    if (!(sh & 1)) {
+                        asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(wbase + 16u * k2), "f"(f0), "f"(f1) : "memory");
+                        asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(wbase + 16u * k2 + 8u), "f"(f2), "f"(f3) : "memory");
+                    } else {
+                        asm volatile("st.shared.f32 [%0], %1;\n" ::"r"(wbase + 16u * k2), "f"(f0) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;\n" ::"r"(wbase + 16u * k2 + 4u), "f"(f1) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;\n" ::"r"(wbase + 16u * k2 + 8u), "f"(f2) : "memory");
+                        asm volatile("st.shared.f32 [%0], %1;\n" ::"r"(wbase + 16u * k2 + 12u), "f"(f3) : "memory");
+                    }
+                }
+            } else if (!(sh & 1)) {
 #pragma unroll
                 for (int k2 = 0; k2 < SB_K / 2; ++k2)
                     asm volatile("st.shared.b64 [%0], %1;\n" ::"r"(wbase + 8u * k2), "l"(acc[j][k2]) : "memory");
@@ -728,7 +821,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
             auto put = [&](int w) {                              // one buffer word, bounds-checked
                 const int sidx = w - sh;
                 const long long tt = t0 + sidx;
-                if (sidx >= 0 && sidx < SB_T && tt >= 0 && tt < A.nsamp_out) {
+                if (sidx >= 0 && sidx < TT && tt >= 0 && tt < A.nsamp_out) {
                     if (first) orow[tt] = ep[w];
                     else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(orow + tt), "f"(ep[w]) : "memory");
                 }
@@ -737,10 +830,10 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                 // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
                 // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
 #pragma unroll 1
-                for (int g = lane; g < (SB_T + 3 + 3) / 4; g += 32) {
+                for (int g = lane; g < (TT + 3 + 3) / 4; g += 32) {
                     const int sidx = 4 * g - sh;
                     const long long tt = t0 + sidx;
-                    if (sidx >= 0 && sidx + 3 < SB_T && tt >= 0 && tt + 3 < A.nsamp_out) {
+                    if (sidx >= 0 && sidx + 3 < TT && tt >= 0 && tt + 3 < A.nsamp_out) {
                         float4 v;
                         asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(ep_u32 + 16u * g));
                         if (first) *reinterpret_cast<float4 *>(orow + tt) = v;
@@ -752,7 +845,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                 }
             } else {
 #pragma unroll 1
-                for (int i = 0; i < SB_K; ++i) put(i * 32 + lane);
+                for (int i = 0; i < TT / 32; ++i) put(i * 32 + lane);
             }
         }
     }
@@ -792,7 +885,8 @@ cudaError_t subband_upload(dedisp_plan *p) {
     if (e != cudaSuccess) return e;
     switch (p->dtype) {
         case DEDISP_U8:
-            e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
+            e = sb.i16 ? cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw)
+                       : cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
             if (e == cudaSuccess && p->time_major) {   // time-major launches use the direct path's layout (no raw buffer)
                 e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
                 if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
@@ -819,7 +913,7 @@ void subband_free(dedisp_plan *p) {
     p->sb.d_passes = nullptr;
 }
 
-bool subband_smem_fits(const dedisp_plan *p) { return sb_smem_bytes(SB_CB, p->sb.max_nch + 1, dtype_esize(p->dtype)) <= 227u * 1024u; }
+bool subband_smem_fits(const dedisp_plan *p) { return sb_smem_bytes(SB_CB, p->sb.max_nch + 1, dtype_esize(p->dtype), p->sb.i16) <= 227u * 1024u; }
 
 // fp32 rows whose base and pitches are 16-byte aligned go straight into the ring; everything else takes the
 // raw path (TMA of the raw bytes + conversion / realignment by the producer warps)
@@ -882,7 +976,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     if (run.tm_bits && (A.cb != 16 || !p->time_major)) return cudaErrorInvalidValue;
     auto tiles_of = [&](const SubbandPass &ps) -> long long {
         const long long nb = std::min(blk_hi, ps.blk_end) - std::max(blk_lo, ps.blk_begin);
-        return nb <= 0 ? 0 : nb * ((nsamp_out + ps.max_skew + SB_T - 1) / SB_T) * b.n;
+        return nb <= 0 ? 0 : nb * ((nsamp_out + ps.max_skew + sb.tile_t - 1) / sb.tile_t) * b.n;
     };
     auto launch = [&](long long tiles) -> cudaError_t {
         if (tiles <= 0) return cudaSuccess;
@@ -894,6 +988,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         else if (run.tm_bits == 2) dedisp_subband_kernel<uint8_t, 4><<<grid, SB_THREADS, sb.smem, st>>>(A);
         else if (run.tm_bits == 1) dedisp_subband_kernel<uint8_t, 5><<<grid, SB_THREADS, sb.smem, st>>>(A);
         else if (!raw) dedisp_subband_kernel<float, 0><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        else if (sb.i16) dedisp_subband_kernel<uint8_t, 6><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
         else if (p->dtype == DEDISP_U8) dedisp_subband_kernel<uint8_t, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
         else if (p->dtype == DEDISP_F16) dedisp_subband_kernel<__half, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);
         else dedisp_subband_kernel<float, 1><<<grid, SB_THREADS, sb.smem_raw, st>>>(A);

@@ -117,6 +117,25 @@ def test_generated_channel_body_is_up_to_date():
         plan_h = f.read()
     assert f"#define SB_D_CFG {d}" in plan_h and f"#define SB_K_CFG {k}" in plan_h
     assert f"#define SB_S_CFG {sp}" in plan_h and f"#define SB_G_CFG {g}" in plan_h
+    # the packed 16-bit variant of u8 plans
+    with open(os.path.join(csrc, "subband_rows_i16.inc")) as f:
+        committed = f.read()
+    d16, k16, omax, stride16 = (int(x) for x in committed.splitlines()[0].split("generate_i16")[1].split(")")[0].split())
+    assert (d16, k16, stride16) == (d, k, stride) and (d16, k16, omax, stride16) == gen.DEFAULT_I16
+    assert committed == gen.generate_i16(d16, k16, omax, stride16)
+    assert f"constexpr int SB16_OMAX = {omax};" in plan_h
+
+
+@pytest.mark.parametrize("name", ["c2", "c5"])
+def test_u8_plans_are_packed_with_at_most_257_channels_per_pass(name):
+    """u8 plans sum packed 16-bit pairs: 257 channels x 255 is the most a 16-bit lane holds, so no pass may be
+    wider; DEDISP_PLAN_NO_PACKED plans keep the fp32 geometry. Both encode the shift table exactly."""
+    cfg = CONFIGS[name]
+    packed = P.Plan.from_config(cfg, host_only=True)
+    plain = P.Plan.from_config(cfg, host_only=True, packed=False)
+    assert packed.verify_records() == 0 and plain.verify_records() == 0      # includes the 257-channel check
+    assert packed.num_subbands() * 257 >= cfg.nchans
+    assert packed.geometry() != plain.geometry()
 
 
 def test_kernel_selection_falls_back_when_subband_is_not_admitted():

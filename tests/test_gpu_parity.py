@@ -344,3 +344,44 @@ def test_merged_passes_match_oracle(name):
         out = plan.execute(x, cfg.nsamp_out)
         torch.cuda.synchronize()
         assert_matches_oracle(cfg, out, ref, what=f"{name}/merged")
+
+
+# ---- u8 plans: packed 16-bit sums on the integer pipes (SubbandGeom::i16) vs. the fp32 sums of DEDISP_PLAN_NO_PACKED
+@pytest.mark.parametrize("name", ["c2s", "c5s", "paper", "fine"])
+def test_packed_and_fp32_u8_plans_both_match_oracle(name):
+    cfg = SMALL[name]
+    x, tab, _ = make_case(cfg)
+    ref = oracle_rows(cfg, x.cpu().numpy())
+    outs = []
+    for packed in (True, False):
+        plan = P.Plan.from_config(cfg, packed=packed)
+        plan.set_kernel(P.KERNEL_SUBBAND)
+        out = plan.execute(x, cfg.nsamp_out)
+        torch.cuda.synchronize()
+        assert_matches_oracle(cfg, out, ref, what=f"{name}/packed={packed}")
+        outs.append(out)
+    assert torch.equal(outs[0], outs[1])
+
+
+@pytest.mark.parametrize("value", [255, "random"])
+def test_packed_sums_do_not_overflow_a_16_bit_lane(value):
+    """The worst case of the packed path: a DM plan so fine that only the 257-channel cap cuts the sub-bands,
+    and input that is 255 everywhere (every 16-bit lane of a full pass ends at 65535 = 257 * 255 exactly) or
+    uniform over 0..255."""
+    cfg = SurveyConfig("packed_overflow", 700, 1500.0, -0.1, 64e-6, 3500, ((0.0, 0.02, 101),), "u8", 128.0, 16.0, 20.0, 0, 5)
+    plan = P.Plan.from_config(cfg)
+    plan.set_kernel(P.KERNEL_SUBBAND)
+    assert plan.verify_records() == 0
+    sb = plan.subbands()
+    assert int(np.diff(sb).max()) == 257                       # a full-width pass exists
+    tab = oracle_table(cfg)
+    nsamp_in = cfg.nsamp_out + int(tab.max())
+    if value == "random":
+        x = np.random.default_rng(11).integers(0, 256, size=(cfg.nchans, nsamp_in), dtype=np.uint8)
+    else:
+        x = np.full((cfg.nchans, nsamp_in), 255, dtype=np.uint8)
+    out = plan.execute(torch.from_numpy(x).cuda(), cfg.nsamp_out)
+    torch.cuda.synchronize()
+    assert_matches_oracle(cfg, out, oracle_rows(cfg, x), what=f"packed overflow {value}")
+    if value == 255:
+        assert int(out.min()) == int(out.max()) == 700 * 255
