@@ -278,9 +278,8 @@ static void subband_build_as(dedisp_plan *p, const bool i16) {
 }
 
 void subband_build(dedisp_plan *p) {
-    // u8 plans sum packed 16-bit pairs on the integer pipes (time-major plans keep the fp32 ring their
-    // scatter writes); should that geometry not be admitted, the fp32 one is tried
-    if (p->dtype == DEDISP_U8 && !p->time_major && !(p->flags & DEDISP_PLAN_NO_PACKED)) {
+    // u8 plans sum packed 16-bit pairs on the integer pipes; should that geometry not be admitted, the fp32 one is tried
+    if (p->dtype == DEDISP_U8 && !(p->flags & DEDISP_PLAN_NO_PACKED)) {
         subband_build_as(p, true);
         if (p->sb.ok) return;
     }
@@ -505,13 +504,13 @@ template <> __device__ __forceinline__ float sb_to_f32<__half>(__half v) { retur
 // channel windows of the ring: the corner turn costs no extra pass over the input and no staging buffer.
 template <typename TIN, int MODE>
 __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbArgs A) {
-    constexpr bool I16 = MODE == 6;   // u8 plan summed as packed 16-bit pairs: ring words hold two samples
-    constexpr bool RAW = MODE == 1 || I16;
+    constexpr bool I16 = MODE >= 6;   // u8 plan summed as packed 16-bit pairs: ring words hold two samples (6: raw, 7..10: time-major)
+    constexpr bool RAW = MODE == 1 || MODE == 6;
     constexpr int TT = I16 ? SB16_T : SB_T;                  // u-samples per tile
     constexpr int CS = I16 ? 8 : 4;                          // samples per staged 16-byte chunk
     constexpr int EPW = I16 ? SB16_EP_WORDS : SB_EP_WORDS;   // words of a warp's transpose buffer
     static_assert(!I16 || std::is_same<TIN, uint8_t>::value, "packed sums are for u8 input");
-    constexpr int TMB = MODE == 2 ? 8 : MODE == 3 ? 4 : MODE == 4 ? 2 : MODE == 5 ? 1 : 0;   // time-major: bits per sample
+    constexpr int TMB = MODE == 2 || MODE == 7 ? 8 : MODE == 3 || MODE == 8 ? 4 : MODE == 4 || MODE == 9 ? 2 : MODE == 5 || MODE == 10 ? 1 : 0;   // time-major: bits per sample
     constexpr bool CONV = RAW || TMB != 0;                                                   // producer warps write the ring
     extern __shared__ __align__(16) unsigned char sb_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -553,7 +552,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                     // lane j < n: window of channel c0 + j in time samples [e0, e0 + nw)
                     const int2 mt = lane < n ? __ldg(meta + c0 + lane) : make_int2(0, 0);
                     const long long e0 = t.U0 + mt.x;
-                    const int nw = 4 * mt.y;
+                    const int nw = CS * mt.y;
                     long long t_lo = lane < n ? e0 : (1ll << 62), t_hi = lane < n ? e0 + nw : -(1ll << 62);
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) {
@@ -568,10 +567,48 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                     // lane j keeps channel j's slot address minus its window start, and its window as [lo, lo + nw)
                     // in samples relative to the union's first sample
                     const int lo = (int)(e0 - t_lo);
-                    const unsigned sbase = sdata_base + buf * stage_bytes + lane * slot_bytes - 4u * (unsigned)lo;
+                    const unsigned sbase = sdata_base + buf * stage_bytes + lane * slot_bytes - (I16 ? 2u : 4u) * (unsigned)lo;
                     const size_t col = (size_t)c0 * TMB / 8;                  // byte of channel c0 in a row
                     constexpr int NW = TMB == 8 ? 4 : TMB == 4 ? 2 : 1;       // 32-bit words per row: 16 channels
                     constexpr int NB = TMB == 8 ? 2 : 4;                      // rows per lane in flight: all loads first, then the scatter
+                    if constexpr (I16) {
+                        // packed ring: a lane takes PAIRS of consecutive time samples (window starts are even: multiples
+                        // of 8 samples), so one 32-bit store per channel covers two samples
+                        constexpr int NP2 = NB / 2 > 0 ? NB / 2 : 1;          // sample pairs per lane in flight
+                        for (long long tb = t_lo + 64 * NP2 * pw; tb < t_hi; tb += 256 * NP2) {
+                            unsigned w[NP2][2][NW];
+#pragma unroll
+                            for (int r = 0; r < NP2; ++r)
+#pragma unroll
+                                for (int h = 0; h < 2; ++h) {
+                                    const long long ts = tb + 64 * r + 2 * lane + h;
+#pragma unroll
+                                    for (int q = 0; q < NW; ++q) w[r][h][q] = 0u;
+                                    if (ts >= 0 && ts < A.in_total && ts < t_hi) {
+                                        const unsigned char *src = inb + (size_t)ts * A.in_stride + col;
+                                        if constexpr (TMB == 8) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(src)); w[r][h][0] = v.x; w[r][h][1] = v.y; w[r][h][2] = v.z; w[r][h][3] = v.w; }
+                                        else if constexpr (TMB == 4) { const uint2 v = __ldg(reinterpret_cast<const uint2 *>(src)); w[r][h][0] = v.x; w[r][h][1] = v.y; }
+                                        else if constexpr (TMB == 2) w[r][h][0] = __ldg(reinterpret_cast<const unsigned *>(src));
+                                        else w[r][h][0] = __ldg(reinterpret_cast<const unsigned short *>(src));
+                                    }
+                                }
+                            const int idx0 = (int)(tb - t_lo) + 2 * lane;
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) {
+                                constexpr unsigned per = 32 / TMB;
+                                const int loj = __shfl_sync(0xffffffffu, lo, j);
+                                const int nj = __shfl_sync(0xffffffffu, nw, j);
+                                const unsigned bj = __shfl_sync(0xffffffffu, sbase, j) + 2u * (unsigned)idx0;
+#pragma unroll
+                                for (int r = 0; r < NP2; ++r) {
+                                    const unsigned x0 = (w[r][0][j / per] >> ((j % per) * TMB)) & ((1u << TMB) - 1u);
+                                    const unsigned x1 = (w[r][1][j / per] >> ((j % per) * TMB)) & ((1u << TMB) - 1u);
+                                    if ((unsigned)(idx0 + 64 * r - loj) < (unsigned)nj)
+                                        asm volatile("st.shared.b32 [%0], %1;\n" ::"r"(bj + 128u * r), "r"(x0 | (x1 << 16)) : "memory");
+                                }
+                            }
+                        }
+                    } else
                     for (long long tb = t_lo + 32 * NB * pw; tb < t_hi; tb += 128 * NB) {   // 32 * NB time samples per warp and step
                         unsigned w[NB][NW];
 #pragma unroll
@@ -887,7 +924,12 @@ cudaError_t subband_upload(dedisp_plan *p) {
         case DEDISP_U8:
             e = sb.i16 ? cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw)
                        : cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem_raw);
-            if (e == cudaSuccess && p->time_major) {   // time-major launches use the direct path's layout (no raw buffer)
+            if (e == cudaSuccess && p->time_major && sb.i16) {
+                e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+                if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
+            } else if (e == cudaSuccess && p->time_major) {   // time-major launches use the direct path's layout (no raw buffer)
                 e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
                 if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
                 if (e == cudaSuccess) e = cudaFuncSetAttribute(dedisp_subband_kernel<uint8_t, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb.smem);
@@ -983,7 +1025,13 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         if (tiles >= (1ll << 31)) return cudaErrorInvalidValue;
         const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, p->sm_count));
         // u8 plans too accumulate fp32 sums (exact, checked at plan build) in place; converted after the last pass
-        if (run.tm_bits == 8) dedisp_subband_kernel<uint8_t, 2><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        if (run.tm_bits && sb.i16) {
+            if (run.tm_bits == 8) dedisp_subband_kernel<uint8_t, 7><<<grid, SB_THREADS, sb.smem, st>>>(A);
+            else if (run.tm_bits == 4) dedisp_subband_kernel<uint8_t, 8><<<grid, SB_THREADS, sb.smem, st>>>(A);
+            else if (run.tm_bits == 2) dedisp_subband_kernel<uint8_t, 9><<<grid, SB_THREADS, sb.smem, st>>>(A);
+            else dedisp_subband_kernel<uint8_t, 10><<<grid, SB_THREADS, sb.smem, st>>>(A);
+        }
+        else if (run.tm_bits == 8) dedisp_subband_kernel<uint8_t, 2><<<grid, SB_THREADS, sb.smem, st>>>(A);
         else if (run.tm_bits == 4) dedisp_subband_kernel<uint8_t, 3><<<grid, SB_THREADS, sb.smem, st>>>(A);
         else if (run.tm_bits == 2) dedisp_subband_kernel<uint8_t, 4><<<grid, SB_THREADS, sb.smem, st>>>(A);
         else if (run.tm_bits == 1) dedisp_subband_kernel<uint8_t, 5><<<grid, SB_THREADS, sb.smem, st>>>(A);

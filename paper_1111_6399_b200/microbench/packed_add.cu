@@ -7,6 +7,9 @@
 //   2  u16x2, even offsets: 26 IADD per row and channel (52 samples)
 //   3  u16x2, odd offsets : 26 funnel-shift+add (one LEA.HI in SASS) per row and channel (52 samples)
 //   4  u16x2, rows alternate even / odd
+//   5  u16x2, even offsets with add.u16x2 (SASS VIADD.16x2)
+//   6  u16x2, even offsets with mad.lo.u32 x, one, acc (SASS IMAD; ptxas turns add.u32 into IMAD.IADD inside the kernel's bodies)
+//   7  u16x2, rows alternate add.u16x2 / funnel-shift+add
 // Build + run: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -o /tmp/packed_add paper_1111_6399_b200/microbench/packed_add.cu && /tmp/packed_add
 #include <cstdio>
 #include <cuda_runtime.h>
@@ -18,6 +21,7 @@ template <int MODE> __global__ void __launch_bounds__(384, 1) k(unsigned *out, i
     for (int i = threadIdx.x; i < 16384; i += blockDim.x) sm[i] = (i * 2654435761u) & 0x00ff00ffu;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned one = nchan > 0 ? 1u : 3u;   // a 1 the compiler cannot see: keeps mode 6 an IMAD
     unsigned acc[D][K];
 #pragma unroll
     for (int j = 0; j < D; ++j)
@@ -47,6 +51,12 @@ template <int MODE> __global__ void __launch_bounds__(384, 1) k(unsigned *out, i
             } else if (MODE == 2 || (MODE == 4 && (j & 1) == 0)) {
 #pragma unroll
                 for (int i = 0; i < K; ++i) asm volatile("add.u32 %0, %0, %1;" : "+r"(acc[j][i]) : "r"(w[i + o]));
+            } else if (MODE == 5 || (MODE == 7 && (j & 1) == 0)) {
+#pragma unroll
+                for (int i = 0; i < K; ++i) asm volatile("add.u16x2 %0, %0, %1;" : "+r"(acc[j][i]) : "r"(w[i + o]));
+            } else if (MODE == 6) {
+#pragma unroll
+                for (int i = 0; i < K; ++i) asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc[j][i]) : "r"(w[i + o]), "r"(one));
             } else {
 #pragma unroll
                 for (int i = 0; i < K; ++i) asm volatile("{.reg .b32 t; shf.r.wrap.b32 t, %1, %2, 16; add.u32 %0, %0, t;}" : "+r"(acc[j][i]) : "r"(w[i + o]), "r"(w[i + o + 1]));
@@ -68,8 +78,8 @@ int main() {
     const int nchan = 200000;
     const double clk = pr.clockRate * 1e3;
     printf("SMs %d clock %d kHz, %d channels, 12 warps/SM\n", pr.multiProcessorCount, pr.clockRate, nchan);
-    const char *name[5] = {"fp32 even (FADD2)", "fp32 odd (FADD)", "u16x2 even (IADD)", "u16x2 odd (LEA.HI)", "u16x2 mixed"};
-    for (int mode = 0; mode < 5; ++mode) {
+    const char *name[8] = {"fp32 even (FADD2)", "fp32 odd (FADD)", "u16x2 even (IADD)", "u16x2 odd (LEA.HI)", "u16x2 mixed", "u16x2 even (VIADD.16x2)", "u16x2 even (IMAD)", "u16x2 mixed VIADD/LEA"};
+    for (int mode = 0; mode < 8; ++mode) {
         float ms = 0;
         for (int rep = 0; rep < 3; ++rep) {
             cudaEventRecord(e0);
@@ -77,6 +87,9 @@ int main() {
             if (mode == 1) { CK(cudaFuncSetAttribute(k<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<1><<<148, 384, 65536>>>(d, nchan); }
             if (mode == 2) { CK(cudaFuncSetAttribute(k<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<2><<<148, 384, 65536>>>(d, nchan); }
             if (mode == 3) { CK(cudaFuncSetAttribute(k<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<3><<<148, 384, 65536>>>(d, nchan); }
+            if (mode == 5) { CK(cudaFuncSetAttribute(k<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<5><<<148, 384, 65536>>>(d, nchan); }
+            if (mode == 6) { CK(cudaFuncSetAttribute(k<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<6><<<148, 384, 65536>>>(d, nchan); }
+            if (mode == 7) { CK(cudaFuncSetAttribute(k<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<7><<<148, 384, 65536>>>(d, nchan); }
             if (mode == 4) { CK(cudaFuncSetAttribute(k<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536)); k<4><<<148, 384, 65536>>>(d, nchan); }
             cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms, e0, e1);
         }
