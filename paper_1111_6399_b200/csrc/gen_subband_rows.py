@@ -221,7 +221,7 @@ def generate_i16(D, K, OMAX, rec_stride):
 
 
 DEFAULT = (4, 26, 5, 2, 96)
-DEFAULT_I16 = (4, 26, 11, 96)
+DEFAULT_I16 = (4, 26, int(os.environ.get('SB16_OMAX', '11')), 96)
 
 if __name__ == "__main__":
     a = [int(x) for x in sys.argv[1:]]

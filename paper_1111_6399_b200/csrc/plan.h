@@ -64,7 +64,10 @@ constexpr int SB_NCH_MAX = ((SB_K * 31 + 2 * SB_WPAIRS + 3) / 4 + 96 + 31) / 32 
 // (profiles/r2_microbench.md, packed_add.cu). Offsets are in samples; window bases stay 8 bytes = 4 samples apart.
 constexpr int SB16_KS = 2 * SB_K;         // samples per thread and row
 constexpr int SB16_T = 32 * SB16_KS;      // u-samples per CTA tile
-constexpr int SB16_OMAX = 11;             // largest in-window offset: word offset 5 + the half-word bit
+#ifndef SB16_OMAX_CFG
+#define SB16_OMAX_CFG 11
+#endif
+constexpr int SB16_OMAX = SB16_OMAX_CFG;  // largest in-window offset (11: word offset 5 + the half-word bit)
 constexpr int SB16_S = SB16_OMAX - 3;     // spread bound of a thread's rows (the smallest offset is 0..3)
 constexpr int SB16_CHMAX = 257;           // channels per pass: 257 * 255 = 65535 still fits a 16-bit lane
 constexpr int SB16_EP_WORDS = SB16_T + 8;

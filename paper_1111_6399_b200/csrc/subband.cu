@@ -890,12 +890,19 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
 
 // u8 plans: the passes accumulate exact fp32 sums in place in the caller's int32 buffer (so that every
 // pass can use the vector reduction); this turns the finished rows into int32, in place.
+// VEC: rows start on 16-byte boundaries, a thread converts four consecutive samples with one 16-byte load and store.
+template <bool VEC>
 __global__ void __launch_bounds__(256) dedisp_f32_to_i32_inplace_kernel(int *__restrict__ out, long long out_stride, long long out_beam,
                                                                           long long nsamp_out, int d0) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * (VEC ? 4 : 1);
     if (i >= nsamp_out) return;
     int *pv = out + (size_t)blockIdx.z * out_beam + (size_t)(d0 + blockIdx.y) * out_stride + i;
-    *pv = __float2int_rn(__int_as_float(*pv));
+    if (VEC && i + 3 < nsamp_out) {
+        const float4 v = *reinterpret_cast<const float4 *>(pv);
+        *reinterpret_cast<int4 *>(pv) = make_int4(__float2int_rn(v.x), __float2int_rn(v.y), __float2int_rn(v.z), __float2int_rn(v.w));
+    } else {
+        for (int q = 0; q < (VEC ? 4 : 1) && i + q < nsamp_out; ++q) pv[q] = __float2int_rn(__int_as_float(pv[q]));
+    }
 }
 
 }  // namespace
@@ -1073,8 +1080,10 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
     if (p->dtype == DEDISP_U8 && pass_hi == nlaunch) {   // last pass done for these rows
         const int d0 = std::min(p->ndm, blk_lo * SB_ROWS), d1 = std::min(p->ndm, blk_hi * SB_ROWS);
         for (int r0 = d0; r0 < d1; r0 += 32768) {   // grid.y <= 65535
-            dim3 grid((unsigned)((nsamp_out + 255) / 256), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
-            dedisp_f32_to_i32_inplace_kernel<<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
+            const int per = A.out_vec4 ? 1024 : 256;   // samples per CTA
+            dim3 grid((unsigned)((nsamp_out + per - 1) / per), (unsigned)std::min(32768, d1 - r0), (unsigned)b.n);
+            if (A.out_vec4) dedisp_f32_to_i32_inplace_kernel<true><<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
+            else dedisp_f32_to_i32_inplace_kernel<false><<<grid, 256, 0, st>>>((int *)d_out, out_stride, b.out_stride, nsamp_out, r0);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
         }

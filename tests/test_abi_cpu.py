@@ -123,7 +123,7 @@ def test_generated_channel_body_is_up_to_date():
     d16, k16, omax, stride16 = (int(x) for x in committed.splitlines()[0].split("generate_i16")[1].split(")")[0].split())
     assert (d16, k16, stride16) == (d, k, stride) and (d16, k16, omax, stride16) == gen.DEFAULT_I16
     assert committed == gen.generate_i16(d16, k16, omax, stride16)
-    assert f"constexpr int SB16_OMAX = {omax};" in plan_h
+    assert f"#define SB16_OMAX_CFG {omax}" in plan_h
 
 
 @pytest.mark.parametrize("name", ["c2", "c5"])
