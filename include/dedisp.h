@@ -38,7 +38,8 @@ enum dedisp_status {
     DEDISP_EINVAL = 1,       /* bad argument (see each call) */
     DEDISP_ENOMEM = 2,       /* host or device allocation failed */
     DEDISP_ECUDA = 3,        /* a CUDA call failed; text via dedisp_last_cuda_error */
-    DEDISP_EUNSUPPORTED = 4  /* device is not sm_100, or maxshift >= 2^31, or plan is host-only */
+    DEDISP_EUNSUPPORTED = 4, /* device is not sm_100, or maxshift >= 2^31, or plan is host-only */
+    DEDISP_ETOOLARGE = 5     /* a size exceeds the fixed scratch of a no-allocation entry point (dedisp_detect_static) */
 };
 
 /* Kernel selection (dedisp_plan_set_kernel). AUTO picks SUBBAND when the plan admits it and its passes
@@ -205,6 +206,28 @@ typedef struct dedisp_candidate {
 long long dedisp_detect_workspace_bytes(int ndm);
 int dedisp_detect(const void *d_block, int block_is_float, int ndm, long long nsamp, long long stride, int nwidths,
                   double threshold, dedisp_candidate *d_cands, long long max_cands, void *d_work, void *stream);
+
+/* dedisp_detect_static: dedisp_detect for callers that cannot call cudaMalloc and have no scratch buffer to hand
+ * over (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation). Same definition,
+ * same kernels, same results as dedisp_detect; the per-row scratch ({S1, S2}, 16 bytes per DM row) lives in a
+ * file-scope `static __device__` array inside the library: DEDISP_DETECT_STATIC_MAX_NDM rows = 128 KB, which
+ * every GPU that loads the library holds until the process exits. The caller still owns inputs and outputs:
+ * d_block and d_cands as for dedisp_detect, and d_count (device, 8-byte aligned, 8 bytes), which holds the total
+ * number of candidates once the call's work on `stream` has completed.
+ * Calls no cudaMalloc / cudaFree / allocating library routine: two cudaMemsetAsync (the scratch rows of this
+ * call and *d_count start at zero; the array otherwise keeps the previous call's contents) and two kernel
+ * launches on `stream`. The first call on each device also looks the array's device address up
+ * (cudaGetSymbolAddress, with that device current; later calls reuse it), so make one call outside a graph
+ * capture first.
+ * ALL calls on a device share the one array: calls that overlap on the GPU (different streams, or different
+ * threads or processes' streams of one context) race and give wrong statistics; serialise them on one stream
+ * or with events, or use dedisp_detect with one workspace per stream.
+ * ETOOLARGE: ndm > DEDISP_DETECT_STATIC_MAX_NDM (nothing is launched). EINVAL: as dedisp_detect, or d_count
+ * NULL / misaligned. ECUDA: a CUDA call failed. */
+#define DEDISP_DETECT_STATIC_MAX_NDM 8192
+int dedisp_detect_static(const void *d_block, int block_is_float, int ndm, long long nsamp, long long stride, int nwidths,
+                         double threshold, dedisp_candidate *d_cands, long long max_cands, unsigned long long *d_count,
+                         void *stream);
 
 const char *dedisp_error_string(int code);
 const char *dedisp_last_cuda_error(const dedisp_plan *plan);

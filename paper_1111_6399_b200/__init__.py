@@ -6,4 +6,4 @@ package is its thin ctypes binding plus the config/synthetic-input modules.
 """
 from .configs import CONFIGS, SurveyConfig, shrink, paper_sweep  # noqa: F401
 from .api import (Plan, Stream, DedispError, shift_table_host, lib,  # noqa: F401,E402
-                  KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND, detect, CAND_DTYPE)
+                  KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND, detect, detect_static, CAND_DTYPE)

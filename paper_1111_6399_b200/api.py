@@ -15,7 +15,8 @@ import torch
 
 from . import build as _build
 
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ETOOLARGE = 0, 1, 2, 3, 4, 5
+DETECT_STATIC_MAX_NDM = 8192   # DEDISP_DETECT_STATIC_MAX_NDM
 U8, F16, F32 = 0, 1, 2
 KERNEL_AUTO, KERNEL_NAIVE, KERNEL_TILED, KERNEL_SUBBAND = 0, 1, 2, 3
 PLAN_HOST_ONLY = 1
@@ -32,7 +33,7 @@ SYMBOLS = (
     "dedisp_execute_strided", "dedisp_execute_batched", "dedisp_execute_host", "dedisp_execute_time_major", "dedisp_plan_destroy", "dedisp_plan_max_shift",
     "dedisp_plan_nchans", "dedisp_plan_ndm", "dedisp_plan_get_shifts", "dedisp_plan_set_kernel",
     "dedisp_plan_get_kernel", "dedisp_plan_set_pass_merge", "dedisp_plan_num_subbands", "dedisp_plan_get_subbands",
-    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_detect_workspace_bytes", "dedisp_detect", "dedisp_error_string",
+    "dedisp_plan_verify_records", "dedisp_plan_launches_per_execute", "dedisp_plan_last_host_slabs", "dedisp_plan_get_geometry", "dedisp_detect_workspace_bytes", "dedisp_detect", "dedisp_detect_static", "dedisp_error_string",
     "dedisp_last_cuda_error", "dedisp_stream_create", "dedisp_stream_push", "dedisp_stream_wait_event", "dedisp_stream_release_after", "dedisp_stream_sync",
     "dedisp_stream_destroy",
 )
@@ -75,6 +76,7 @@ def lib() -> ctypes.CDLL:
         L.dedisp_detect_workspace_bytes.argtypes = [c_int]
         L.dedisp_detect_workspace_bytes.restype = c_ll
         L.dedisp_detect.argtypes = [vp, c_int, c_int, c_ll, c_ll, c_int, c_dbl, vp, c_ll, vp, vp]
+        L.dedisp_detect_static.argtypes = [vp, c_int, c_int, c_ll, c_ll, c_int, c_dbl, vp, c_ll, vp, vp]
         L.dedisp_plan_verify_records.argtypes = [vp]
         L.dedisp_plan_verify_records.restype = c_ll
         L.dedisp_error_string.argtypes = [c_int]
@@ -323,4 +325,29 @@ def detect(block: torch.Tensor, nwidths: int, threshold: float, max_cands: int =
     torch.cuda.synchronize(block.device)
     total = int(work[0].item())
     out = np.frombuffer(cands[:min(total, max_cands) * CAND_DTYPE.itemsize].cpu().numpy().tobytes(), dtype=CAND_DTYPE)
+    return out, total
+
+
+def detect_static(block: torch.Tensor, nwidths: int, threshold: float, max_cands: int = 1 << 20, stream=None,
+                  cands: Optional[torch.Tensor] = None, count: Optional[torch.Tensor] = None):
+    """``dedisp_detect_static``: ``detect`` without a workspace - the library call allocates nothing, its scratch is a
+    fixed ``static __device__`` array (at most DETECT_STATIC_MAX_NDM rows; calls that overlap on the GPU race).
+    The outputs are the caller's: pass ``cands`` (uint8, >= max_cands records) and ``count`` (int64[1]) to reuse
+    buffers, else they are made here. Returns (candidates as a CAND_DTYPE numpy array, total count)."""
+    assert block.is_cuda and block.dim() == 2 and block.stride(1) == 1 and block.dtype in (torch.int32, torch.float32)
+    ndm, nsamp = block.shape
+    if cands is None:
+        cands = torch.empty(max(1, max_cands) * CAND_DTYPE.itemsize, dtype=torch.uint8, device=block.device)
+    if count is None:
+        count = torch.empty(1, dtype=torch.int64, device=block.device)
+    assert cands.is_cuda and cands.numel() * cands.element_size() >= max_cands * CAND_DTYPE.itemsize
+    assert count.is_cuda and count.dtype == torch.int64 and count.numel() >= 1
+    rc = lib().dedisp_detect_static(block.data_ptr(), int(block.dtype == torch.float32), ndm, nsamp, block.stride(0), int(nwidths),
+                                    float(threshold), cands.data_ptr(), int(max_cands), count.data_ptr(), _stream_ptr(stream))
+    if rc:
+        raise DedispError(rc, "dedisp_detect_static")
+    torch.cuda.synchronize(block.device)
+    total = int(count[0].item())
+    flat = cands.view(torch.uint8).reshape(-1)
+    out = np.frombuffer(flat[:min(total, max_cands) * CAND_DTYPE.itemsize].cpu().numpy().tobytes(), dtype=CAND_DTYPE)
     return out, total

@@ -13,6 +13,7 @@
 // neighbouring warp segments overlap by the largest width, served by L1/L2); roofline = 2 x block bytes /
 // HBM bandwidth.
 #include <cstdint>
+#include <mutex>
 #include <type_traits>
 
 #include "plan.h"
@@ -210,3 +211,63 @@ int dedisp_detect(const void *d_block, int block_is_float, int ndm, long long ns
 }
 
 }  // extern "C"
+
+// =====================================================================================
+// dedisp_detect_static: the same two kernels for callers that cannot provide (or allocate) scratch memory
+// =====================================================================================
+namespace {
+
+// Scratch of dedisp_detect_static: {S1, S2} of every DM row. 128 KB that every GPU which loads the library holds
+// until the process exits. In HOST code this name is a host-side stand-in, not a device address: the address the
+// kernels get is looked up once per device with cudaGetSymbolAddress (det_static_scratch below).
+static __device__ __align__(256) unsigned long long det_static_stats[2 * DEDISP_DETECT_STATIC_MAX_NDM];
+
+constexpr int DET_MAX_DEVICES = 64;
+std::mutex det_static_mu;
+unsigned long long *det_static_addr[DET_MAX_DEVICES];   // device address of det_static_stats on device i, NULL: not looked up yet
+
+// Device address of the static scratch on the CURRENT device (set-up: once per device, with that device current).
+cudaError_t det_static_scratch(unsigned long long **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= DET_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(det_static_mu);
+    if (!det_static_addr[dev]) {
+        unsigned long long *ptr = nullptr;
+        e = cudaGetSymbolAddress((void **)&ptr, det_static_stats);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        det_static_addr[dev] = ptr;
+    }
+    *out = det_static_addr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int dedisp_detect_static(const void *d_block, int block_is_float, int ndm, long long nsamp, long long stride, int nwidths,
+                                    double threshold, dedisp_candidate *d_cands, long long max_cands, unsigned long long *d_count,
+                                    void *stream) {
+    if (!d_block || !d_count || ((uintptr_t)d_count & 7) || ndm < 1 || nsamp < 1 || stride < nsamp || max_cands < 0 || (max_cands && !d_cands))
+        return DEDISP_EINVAL;
+    if (nwidths < 1 || nwidths > DEDISP_DETECT_MAX_WIDTHS) return DEDISP_EINVAL;
+    if (ndm > DEDISP_DETECT_STATIC_MAX_NDM) return DEDISP_ETOOLARGE;   // the static scratch holds no more rows
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long *stats = nullptr;
+    if (det_static_scratch(&stats) != cudaSuccess) return DEDISP_ECUDA;
+    // the array keeps the last call's sums, and the sums are accumulated with atomics: clear the rows of this call
+    cudaError_t e = cudaMemsetAsync(stats, 0, (size_t)ndm * 16, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_count, 0, 8, st);
+    if (e != cudaSuccess) return DEDISP_ECUDA;
+    const long long per2 = (long long)det_own(nwidths) * (DET_THREADS / 32) * DET_SEGS;
+    const dim3 g1((unsigned)((nsamp + DET_TILE * 8 - 1) / (DET_TILE * 8)), (unsigned)ndm), g2((unsigned)((nsamp + per2 - 1) / per2), (unsigned)ndm);
+    if (block_is_float) {
+        dedisp_detect_stats_kernel<float><<<g1, DET_THREADS, 0, st>>>((const float *)d_block, stride, nsamp, stats);
+        dedisp_detect_boxcar_kernel<float><<<g2, DET_THREADS, 0, st>>>((const float *)d_block, stride, nsamp, nwidths, threshold, stats, d_cands, max_cands, d_count);
+    } else {
+        dedisp_detect_stats_kernel<int><<<g1, DET_THREADS, 0, st>>>((const int *)d_block, stride, nsamp, stats);
+        dedisp_detect_boxcar_kernel<int><<<g2, DET_THREADS, 0, st>>>((const int *)d_block, stride, nsamp, nwidths, threshold, stats, d_cands, max_cands, d_count);
+    }
+    return cudaGetLastError() == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+}

@@ -346,6 +346,7 @@ const char *dedisp_error_string(int code) {
         case DEDISP_ENOMEM: return "out of memory";
         case DEDISP_ECUDA: return "CUDA error";
         case DEDISP_EUNSUPPORTED: return "unsupported (device is not sm_100, shift >= 2^31, host-only plan, or kernel not admitted by the plan)";
+        case DEDISP_ETOOLARGE: return "size exceeds the fixed scratch of a no-allocation entry point (dedisp_detect_static: ndm > DEDISP_DETECT_STATIC_MAX_NDM)";
         default: return "unknown error code";
     }
 }
