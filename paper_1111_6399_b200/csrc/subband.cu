@@ -864,20 +864,42 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
                 }
             };
             if (A.out_vec4) {
-                // 16-byte groups: a plain vector store in the first pass, one fire-and-forget vector
-                // reduction (SASS REDG.E.ADD.F32x4) in the later ones - the SM never waits for out
-#pragma unroll 1
-                for (int g = lane; g < (TT + 3 + 3) / 4; g += 32) {
-                    const int sidx = 4 * g - sh;
-                    const long long tt = t0 + sidx;
-                    if (sidx >= 0 && sidx + 3 < TT && tt >= 0 && tt + 3 < A.nsamp_out) {
-                        float4 v;
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(ep_u32 + 16u * g));
-                        if (first) *reinterpret_cast<float4 *>(orow + tt) = v;
-                        else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
-                                          ::"l"(orow + tt), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-                    } else {
-                        put(4 * g); put(4 * g + 1); put(4 * g + 2); put(4 * g + 3);
+                // Valid buffer words [w_lo, w_hi): inside the tile (w - sh in [0, TT)) and inside the row (t in
+                // [0, nsamp_out)); warp-uniform, found once per row. The whole 16-byte groups [gf_lo, gf_hi) go out
+                // as one LDS.128 + one plain vector store (first pass) or one fire-and-forget vector reduction
+                // (SASS REDG.E.ADD.F32x4; the SM never waits for out) each, NB at a time so that the shared-memory
+                // latencies overlap; the up to 3 + 3 words left over at the two ends go out one by one from lanes 0..7.
+                const long long lo64 = max((long long)sh, (long long)sh - t0), hi64 = min((long long)(sh + TT), A.nsamp_out - t0 + sh);
+                const int w_lo = (int)min(max(lo64, 0ll), (long long)(TT + 8)), w_hi = (int)min(max(hi64, 0ll), (long long)(TT + 8));
+                if (w_hi > w_lo) {
+                    const int gf_lo = (w_lo + 3) >> 2, gf_hi = w_hi >> 2;
+                    const unsigned long long obase = (unsigned long long)orow + 4ull * (unsigned long long)(t0 - sh);   // buffer word w <-> address obase + 4 w
+                    constexpr int NG = (TT + 3 + 3) / 4, NB = 4;
+#pragma unroll
+                    for (int b = 0; b < (NG + 32 * NB - 1) / (32 * NB); ++b) {
+                        float4 v[NB];
+#pragma unroll
+                        for (int q = 0; q < NB; ++q) {
+                            // unconditional load (a group index past the buffer is folded back into it): only valid groups are stored
+                            const int g = lane + 32 * (NB * b + q);
+                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w) : "r"(ep_u32 + 16u * (g < NG ? g : lane)));
+                        }
+#pragma unroll
+                        for (int q = 0; q < NB; ++q) {
+                            const int g = lane + 32 * (NB * b + q);
+                            if (g >= gf_lo && g < gf_hi) {
+                                if (first) *reinterpret_cast<float4 *>(obase + 16ull * g) = v[q];
+                                else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n"
+                                                  ::"l"(obase + 16ull * g), "f"(v[q].x), "f"(v[q].y), "f"(v[q].z), "f"(v[q].w) : "memory");
+                            }
+                        }
+                    }
+                    if (lane < 8) {   // lanes 0..3: the partial group below gf_lo; lanes 4..7: the one at gf_hi (the same group if gf_hi < gf_lo)
+                        const int w = lane < 4 ? 4 * gf_lo - 4 + lane : 4 * gf_hi + lane - 4;
+                        if (w >= w_lo && w < w_hi && (lane < 4 || gf_hi >= gf_lo)) {
+                            if (first) *reinterpret_cast<float *>(obase + 4ull * w) = ep[w];
+                            else asm volatile("red.global.add.f32 [%0], %1;\n" ::"l"(obase + 4ull * w), "f"(ep[w]) : "memory");
+                        }
                     }
                 }
             } else {
