@@ -131,9 +131,10 @@ int dedisp_execute_batched(dedisp_plan *plan, int nbeams, const void *d_in, long
  * maxshift] and h_out [ndm][nsamp_out] are HOST buffers (pinned memory makes the copies
  * asynchronous to the host and full speed). Copies the input to plan-owned device scratch (grown
  * on demand, freed at destroy), executes, copies the result back and SYNCHRONISES `stream` before
- * returning. For the SUBBAND kernel on 16-byte-aligned fp32 rows the input is copied per sub-band
- * pass (smallest first) on a plan-owned second stream, ordered after `stream`, and the result per DM
- * slab of the last pass on a third, so both transfers overlap the passes. Not re-entrant per plan (the scratch is shared). */
+ * returning. For the SUBBAND kernel with more than one launch (any in_dtype) the input is copied in the
+ * order the launches need it (they run last sub-band first, so a growing suffix of the channels) on a
+ * plan-owned second stream, ordered after `stream`, and the result per DM slab of the last two launches on
+ * a third, so both transfers overlap the launches. Not re-entrant per plan (the scratch is shared). */
 int dedisp_execute_host(dedisp_plan *plan, const void *h_in, long long nsamp_out, void *h_out,
                         void *stream);
 
@@ -175,8 +176,8 @@ int dedisp_plan_launches_per_execute(const dedisp_plan *plan);
  * channel window, dynamic shared memory of the two paths, DM blocks, DM ranges, passes}. Zeros if the
  * plan does not admit SUBBAND. */
 int dedisp_plan_get_geometry(const dedisp_plan *plan, int *h_out);
-/* Number of DM slabs the last dedisp_execute_host call on this plan ran its final pass in (0: the
- * call did not take the slab-overlap path). For the tests that must know which path they exercised. */
+/* Number of DM slabs the last dedisp_execute_host call on this plan ran its final pass(es) in (0: the
+ * call did not take the slab-overlap path; else min(8, DM blocks)). For the tests that must know which path they exercised. */
 int dedisp_plan_last_host_slabs(const dedisp_plan *plan);
 
 /* ---- detection behind the hot path ("detect millisecond radio

@@ -171,17 +171,19 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host output scratch");
         p->host_out_bytes = out_bytes;
     }
-    // SUBBAND on aligned fp32 rows reads only the channels of its own sub-band in pass g: copy the
-    // sub-bands in pass order on a second stream and let pass g start as soon as its rows have landed,
-    // so that most of the H2D transfer hides under the earlier passes.
-    const bool overlap = resolve_kernel(p) == DEDISP_KERNEL_SUBBAND && p->dtype == DEDISP_F32 && (nsamp_in & 3) == 0 &&
-                         p->sb.passes.size() > 1 && p->sb.nranges == 1 && !subband_merges(p);   // a merged launch reads every channel at once
+    // A SUBBAND launch reads only the channels of its own sub-bands (plus at most 15 bytes on either side of a
+    // window, which are discarded): copy the channels in the order the launches need them on a second stream
+    // and let launch g start as soon as its rows have landed, so that most of the H2D transfer hides under
+    // the earlier launches. The launches run last sub-band first (fewest channels: the first launch starts
+    // early), so what launch g needs is always a suffix [min c_begin of its passes, nchans) of the channels.
+    const int nlaunch = (int)p->sb.launch_begin.size() - 1;
+    const bool overlap = resolve_kernel(p) == DEDISP_KERNEL_SUBBAND && nlaunch > 1 && !subband_merges(p);   // a merged launch reads every channel at once
     if (overlap) {
         if (!p->host_copy_st) {
             e = cudaStreamCreateWithFlags(&p->host_copy_st, cudaStreamNonBlocking);
             if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host copy stream");
         }
-        while (p->host_pass_ready.size() < p->sb.passes.size()) {
+        while ((int)p->host_pass_ready.size() < nlaunch) {
             cudaEvent_t ev;
             e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
             if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host event");
@@ -190,12 +192,18 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
         cudaEvent_t start = p->host_pass_ready[0];           // order the copy stream after the caller's stream
         e = cudaEventRecord(start, st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_copy_st, start, 0);
-        const size_t row_bytes = (size_t)nsamp_in * sizeof(float);
-        for (size_t i = 0; i < p->sb.passes.size() && e == cudaSuccess; ++i) {
-            const size_t g = p->sb.passes.size() - 1 - i;     // last sub-band first: it has the fewest channels
-            const SubbandPass &ps = p->sb.passes[g];
-            e = cudaMemcpyAsync((char *)p->d_host_in + ps.c_begin * row_bytes, (const char *)h_in + ps.c_begin * row_bytes,
-                                (size_t)(ps.c_end - ps.c_begin) * row_bytes, cudaMemcpyHostToDevice, p->host_copy_st);
+        const size_t row_bytes = (size_t)nsamp_in * dtype_esize(p->dtype);
+        int copied_from = p->nchans;                          // channels [copied_from, nchans) are queued
+        for (int i = 0; i < nlaunch && e == cudaSuccess; ++i) {
+            const int g = nlaunch - 1 - i;
+            int need = p->nchans;
+            for (int q = p->sb.launch_begin[g]; q < p->sb.launch_begin[g + 1]; ++q) need = std::min(need, p->sb.passes[q].c_begin);
+            if (g == 0) need = 0;
+            if (need < copied_from) {
+                e = cudaMemcpyAsync((char *)p->d_host_in + need * row_bytes, (const char *)h_in + need * row_bytes,
+                                    (size_t)(copied_from - need) * row_bytes, cudaMemcpyHostToDevice, p->host_copy_st);
+                copied_from = need;
+            }
             if (e == cudaSuccess) e = cudaEventRecord(p->host_pass_ready[g], p->host_copy_st);
         }
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host H2D");
@@ -211,35 +219,44 @@ int dedisp_execute_host(dedisp_plan *p, const void *h_in, long long nsamp_out, v
     }
     p->host_slabs = 0;
     if (overlap && p->sb.nblk >= 4) {
-        // ... and run the LAST pass slab by slab over the DM blocks, so that the D2H copy of a finished
-        // slab of out rows overlaps the rest of that pass
-        constexpr int NSLAB = 4;
+        // ... and run the LAST TWO passes slab by slab over the DM blocks, so that the D2H copy of a finished
+        // slab of out rows overlaps the rest of the work. Every output row needs every input channel, so no
+        // slab can finish before the H2D copy has: the last pass of the first slab waits for it, and the
+        // second-last pass of LOOKAHEAD further slabs is queued in front of it to fill that wait.
+        const int NSLAB = std::min(8, p->sb.nblk), LOOKAHEAD = 2;
         if (!p->host_d2h_st) e = cudaStreamCreateWithFlags(&p->host_d2h_st, cudaStreamNonBlocking);
-        while (e == cudaSuccess && p->host_slab_done.size() < NSLAB) {
+        while (e == cudaSuccess && (int)p->host_slab_done.size() < NSLAB) {
             cudaEvent_t ev;
             e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
             if (e == cudaSuccess) p->host_slab_done.push_back(ev);
         }
         if (e != cudaSuccess) return fail_cuda(p, e, "dedisp_execute_host slabs");
-        // all passes but the last over the whole grid, then the last pass slab by slab
-        const int npass = (int)p->sb.passes.size();
-        run.pass_lo = 0; run.pass_hi = npass - 1;
+        const int npass = nlaunch;                           // launches, in the order they run
+        const int nslabbed = npass >= 3 ? 2 : 1;             // launches (the last ones to run) done slab by slab
+        run.pass_lo = 0; run.pass_hi = npass - nslabbed;     // the others over the whole grid
         rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, run);
-        run.pass_lo = npass - 1; run.pass_hi = npass;
+        auto slab_pass = [&](int i, int sl) -> int {         // launch-order pass i on DM slab sl
+            SbRun r = run;
+            r.pass_lo = i; r.pass_hi = i + 1;
+            r.blk_lo = (int)((long long)p->sb.nblk * sl / NSLAB);
+            r.blk_hi = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
+            return execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, r);
+        };
+        if (nslabbed == 2)
+            for (int sl = 0; sl < std::min(LOOKAHEAD, NSLAB) && rc == DEDISP_OK; ++sl) rc = slab_pass(npass - 2, sl);
         for (int sl = 0; sl < NSLAB && rc == DEDISP_OK; ++sl) {
-            run.blk_lo = (int)((long long)p->sb.nblk * sl / NSLAB);
-            run.blk_hi = (int)((long long)p->sb.nblk * (sl + 1) / NSLAB);
-            rc = execute_impl(p, p->d_host_in, nsamp_in, nsamp_out, p->d_host_out, nsamp_out, Batch(), st, run);
+            rc = slab_pass(npass - 1, sl);
             if (rc != DEDISP_OK) break;
             ++p->host_slabs;
-            const long long d0 = std::min<long long>(p->ndm, (long long)run.blk_lo * SB_ROWS);
-            const long long d1 = std::min<long long>(p->ndm, (long long)run.blk_hi * SB_ROWS);
+            const long long d0 = std::min<long long>(p->ndm, (long long)((long long)p->sb.nblk * sl / NSLAB) * SB_ROWS);
+            const long long d1 = std::min<long long>(p->ndm, (long long)((long long)p->sb.nblk * (sl + 1) / NSLAB) * SB_ROWS);
             e = cudaEventRecord(p->host_slab_done[sl], st);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(p->host_d2h_st, p->host_slab_done[sl], 0);
             if (e == cudaSuccess && d1 > d0)
                 e = cudaMemcpyAsync((char *)h_out + d0 * nsamp_out * 4, (char *)p->d_host_out + d0 * nsamp_out * 4,
                                     (size_t)(d1 - d0) * nsamp_out * 4, cudaMemcpyDeviceToHost, p->host_d2h_st);
-            if (e != cudaSuccess) rc = fail_cuda(p, e, "dedisp_execute_host slab D2H");
+            if (e != cudaSuccess) { rc = fail_cuda(p, e, "dedisp_execute_host slab D2H"); break; }
+            if (nslabbed == 2 && sl + LOOKAHEAD < NSLAB) rc = slab_pass(npass - 2, sl + LOOKAHEAD);
         }
         if (rc != DEDISP_OK) return rc;
         e = cudaStreamSynchronize(p->host_d2h_st);

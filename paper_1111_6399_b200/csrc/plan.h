@@ -86,7 +86,7 @@ struct SbPassDev {
     int blk_begin, blk_end;
     int max_skew;
     int first;
-    int pad0, pad1;
+    int pad0, pad1;                   // pad0: 1 = last sub-band of its DM range (stores when the launches run in reverse order)
 };
 
 // What one SUBBAND launch sequence covers: launch-order range of passes, DM-block range, order, and

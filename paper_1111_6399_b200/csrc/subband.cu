@@ -414,7 +414,8 @@ struct SbArgs {
     int slot_chunks;          // 16-byte chunks per staged channel slot
     int raw_slot_bytes;       // raw path: bytes per raw channel slot
     int cb;                   // channels per pipeline stage (SB_CB .. SB_CB_MAX)
-    int first;                // 1: the launch's passes store, 0: every pass adds into out, 2: per pass (table flag)
+    int first;                // 1: the launch's passes store, 0: every pass adds into out, 2: per pass (first sub-band of its DM range),
+                              // 3: per pass (last sub-band of its range: launches in reverse order)
     int out_vec4;             // out rows are 16-byte aligned (base, row stride, beam stride): vector epilogue
 };
 
@@ -454,7 +455,7 @@ __device__ __forceinline__ bool sb_next_tile(const SbArgs &A, SbTile &t) {
         if (t.U0 + TT <= (long long)__ldg(t.skew + d_first) || t.U0 >= (long long)__ldg(t.skew + d_last) + A.nsamp_out) continue;
         t.c_begin = P.c_begin;
         t.c_end = P.c_end;
-        t.first = P.first;
+        t.first = A.first == 3 ? P.pad0 : P.first;   // 3: the passes run last sub-band first, so a range's LAST sub-band stores
         return true;
     }
 }
@@ -815,7 +816,7 @@ __global__ void __launch_bounds__(SB_THREADS, 1) dedisp_subband_kernel(const SbA
         // are 16-byte aligned in the buffer too: one LDS.128 + one vector store / reduction per group.
         float *out = reinterpret_cast<float *>(A.out) + (size_t)t.beam * A.out_beam;
         const int d0 = t.blk * SB_ROWS + warp * SB_D;
-        const int first = A.first == 2 ? t.first : A.first;
+        const int first = A.first >= 2 ? t.first : A.first;
         const unsigned ep_u32 = (unsigned)__cvta_generic_to_shared(ep);
 #pragma unroll
         for (int j = 0; j < SB_D; ++j) {
@@ -938,7 +939,9 @@ cudaError_t subband_upload(dedisp_plan *p) {
     std::vector<SbPassDev> tab(sb.passes.size());
     for (size_t g = 0; g < sb.passes.size(); ++g) {
         const SubbandPass &ps = sb.passes[g];
-        tab[g] = SbPassDev{ps.c_begin, ps.c_end, ps.blk_begin, ps.blk_end, ps.max_skew, ps.first ? 1 : 0, 0, 0};
+        bool last = true;                                 // no later pass covers this pass's DM blocks: the last sub-band of its range
+        for (size_t h = g + 1; h < sb.passes.size(); ++h) last = last && sb.passes[h].blk_begin != ps.blk_begin;
+        tab[g] = SbPassDev{ps.c_begin, ps.c_end, ps.blk_begin, ps.blk_end, ps.max_skew, ps.first ? 1 : 0, last ? 1 : 0, 0};
     }
     cudaError_t e = cudaMalloc(&sb.d_records, sb.records.size() * sizeof(uint64_t));
     if (e == cudaSuccess) e = cudaMemcpy(sb.d_records, sb.records.data(), sb.records.size() * sizeof(uint64_t), cudaMemcpyHostToDevice);
@@ -1088,7 +1091,7 @@ cudaError_t launch_subband(dedisp_plan *p, const void *d_in, long long in_stride
         for (int i = run.pass_lo; i < pass_hi; ++i) {
             const int g = run.reverse ? nlaunch - 1 - i : i;          // launch g = passes [launch_begin[g], launch_begin[g + 1])
             A.pass_lo = sb.launch_begin[g]; A.pass_hi = sb.launch_begin[g + 1];
-            A.first = sb.nranges == 1 ? i == 0 : 2;   // one range: any order, the first launched pass stores; else per pass
+            A.first = sb.nranges == 1 ? i == 0 : run.reverse ? 3 : 2;   // one range: any order, the first launched pass stores; else per pass
             if (run.pass_ready) {   // dedisp_execute_host (one DM range): this pass's channel rows arrive on the copy stream
                 e = cudaStreamWaitEvent(st, run.pass_ready[g], 0);
                 if (e != cudaSuccess) return e;

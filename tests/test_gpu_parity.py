@@ -293,14 +293,16 @@ def test_execute_host_matches_oracle(name):
         h_in = x.pin_memory()
         out = plan.execute_host(h_in, cfg.nsamp_out)
         assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"{name}/execute_host seed {seed}")
+    if name == "c4s":   # fp16, three DM ranges: launches in reverse order, each range's last sub-band stores; 4 DM blocks = 4 slabs
+        assert plan.kernel == P.KERNEL_SUBBAND and plan.geometry()["nranges"] == 3 and plan.last_host_slabs == 4
     if name == "c3s":
         assert plan.num_subbands() > 1 and (cfg.nsamp_out + plan.max_shift) % 4 == 0
 
 
 def test_execute_host_slab_branch_matches_oracle():
     """The branch bench.py's e2e figure times on c3: aligned fp32 rows, > 1 pass, >= 4 DM blocks, so
-    that the per-pass H2D overlap AND the last pass in 4 DM slabs with overlapped D2H both run
-    (plan.cu dedisp_execute_host). Full output vs the oracle, twice with different data."""
+    that the per-pass H2D overlap AND the last two passes in DM slabs (one per DM block here, at most 8) with
+    overlapped D2H both run (plan.cu dedisp_execute_host). Full output vs the oracle, twice with different data."""
     cfg = shrink(CONFIGS["c3"], nchans=300, nsamp_out=4500, ndm_stride=16)      # 256 DMs -> 6 DM blocks
     tab = oracle_table(cfg)
     cfg = shrink(cfg, nsamp_out=cfg.nsamp_out + (-(cfg.nsamp_out + int(tab.max())) % 4))
@@ -310,8 +312,22 @@ def test_execute_host_slab_branch_matches_oracle():
     for seed in (21, 22):
         x, _, _ = make_case(cfg, device="cpu", seed=seed)
         out = plan.execute_host(x.pin_memory(), cfg.nsamp_out)
-        assert plan.last_host_slabs == 4, "the slab branch was not taken"
+        assert plan.last_host_slabs == 6, "the slab branch was not taken"
         assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"execute_host slabs seed {seed}")
+
+
+def test_execute_host_slab_branch_u8_unmerged_passes():
+    """The same branch for a u8 plan whose passes are launched one by one (packed 16-bit sums, raw path): the
+    channels arrive in the order the launches need them, the last two launches run slab by slab, and every slab's
+    rows are converted to int32 before their D2H copy. Bit-exact against the oracle, twice."""
+    cfg = SurveyConfig("host_u8", 700, 1500.0, -0.4, 64e-6, 3000, ((0.0, 2.0, 240),), "u8", 128.0, 16.0, 20.0, 1, 9)
+    plan = P.Plan.from_config(cfg)
+    assert plan.kernel == P.KERNEL_SUBBAND and plan.launches_per_execute == plan.num_subbands() + 1 == 7    # 6 passes + the conversion
+    for seed in (31, 32):
+        x, _, _ = make_case(cfg, device="cpu", seed=seed)
+        out = plan.execute_host(x.pin_memory(), cfg.nsamp_out)
+        assert plan.last_host_slabs == 5, "the slab branch was not taken"
+        assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"execute_host u8 slabs seed {seed}")
 
 
 def test_execute_host_with_merged_passes():
