@@ -316,6 +316,24 @@ def test_execute_host_slab_branch_matches_oracle():
         assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"execute_host slabs seed {seed}")
 
 
+def test_execute_host_multi_range_without_slabs():
+    """Three DM ranges in three DM blocks (< 4: no slab overlap): the launches still run last sub-band first with
+    the H2D copy ordered to match, and every range's LAST sub-band stores. Full output vs the oracle, twice."""
+    cfg = shrink(CONFIGS["c4"], nchans=257, nsamp_out=3100, ndm_stride=40)       # 105 DMs: 3 blocks, 3 ranges
+    plan = P.Plan.from_config(cfg)
+    plan.set_kernel(P.KERNEL_SUBBAND)
+    g = plan.geometry()
+    assert g["nblk"] == 3 and g["nranges"] == 3 and plan.launches_per_execute > 1
+    for seed in (41, 42):
+        x, _, _ = make_case(cfg, device="cpu", seed=seed)
+        out = plan.execute_host(x.pin_memory(), cfg.nsamp_out)
+        assert plan.last_host_slabs == 0
+        assert_matches_oracle(cfg, out, oracle_rows(cfg, x.numpy()), what=f"execute_host 3 ranges seed {seed}")
+        dev = plan.execute(x.cuda(), cfg.nsamp_out)                                # forward order, resident input
+        torch.cuda.synchronize()
+        assert_matches_oracle(cfg, dev, oracle_rows(cfg, x.numpy()), what=f"execute 3 ranges seed {seed}")
+
+
 def test_execute_host_slab_branch_u8_unmerged_passes():
     """The same branch for a u8 plan whose passes are launched one by one (packed 16-bit sums, raw path): the
     channels arrive in the order the launches need them, the last two launches run slab by slab, and every slab's
