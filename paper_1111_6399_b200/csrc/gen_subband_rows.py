@@ -215,7 +215,7 @@ def generate_i16(D, K, OMAX, rec_stride):
             "// own offset into %d bodies; the last row's bodies prefetch the next channel's window and jump straight into it.\n"
             % (D, K, OMAX, rec_stride, NP, OMAX + 1))
     params = ("#ifdef SB_ROWS_PARAMS\n"
-              "static_assert(SB_D == %d && SB_K == %d && SB16_OMAX == %d && SB_REC_STRIDE == %d && SB_WPAIRS == %d, \"regenerate subband_rows_i16.inc (gen_subband_rows.py)\");\n"
+              "static_assert(SB_D == %d && SB_K == %d && SB16_OMAX == %d && SB_REC_STRIDE == %d && SB16_WPAIRS == %d, \"regenerate subband_rows_i16.inc (gen_subband_rows.py)\");\n"
               "#else\n" % (D, K, OMAX, rec_stride, NP))
     return head + params + ("asm volatile(\n%s\n    : %s\n    : \"r\"(rp0), \"r\"(slot0), \"r\"(slot_bytes), \"r\"(nch)\n    : \"memory\");\n#endif\n" % (text, outs))
 

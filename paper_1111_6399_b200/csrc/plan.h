@@ -71,7 +71,7 @@ constexpr int SB16_OMAX = SB16_OMAX_CFG;  // largest in-window offset (11: word 
 constexpr int SB16_S = SB16_OMAX - 3;     // spread bound of a thread's rows (the smallest offset is 0..3)
 constexpr int SB16_CHMAX = 257;           // channels per pass: 257 * 255 = 65535 still fits a 16-bit lane
 constexpr int SB16_EP_WORDS = SB16_T + 8;
-static_assert((SB16_OMAX >> 1) + SB_K + 1 <= 2 * SB_WPAIRS, "the packed window must fit the SB_WPAIRS pairs a thread loads");
+constexpr int SB16_WPAIRS = ((SB16_OMAX >> 1) + SB_K + 2) / 2;   // 8-byte pairs a thread loads per channel (its own count: the fp32 loop's may differ)
 
 struct SubbandPass {
     int c_begin = 0, c_end = 0, c_ref = 0;

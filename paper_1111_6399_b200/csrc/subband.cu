@@ -45,7 +45,7 @@ struct SbUnits {
     bool joint;     // record holds joint pattern ids per SB_G rows (fp32) / one offset per row (i16)
 };
 inline SbUnits sb_units(bool i16) {
-    return i16 ? SbUnits{4, 8, SB16_OMAX, SB16_S, SB16_KS, 4 * SB_WPAIRS, 8, SB16_CHMAX, false}
+    return i16 ? SbUnits{4, 8, SB16_OMAX, SB16_S, SB16_KS, 4 * SB16_WPAIRS, 8, SB16_CHMAX, false}
                : SbUnits{2, 4, SB_OMAX, SB_S, SB_K, 2 * SB_WPAIRS, 4, INT32_MAX, true};
 }
 
